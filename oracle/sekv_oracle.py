@@ -363,15 +363,17 @@ def mixed_entries(q_h: np.ndarray, g: int, T: Tables, zoom: Sequence[int]) -> Tu
     return np.concatenate(logits), np.concatenate(values, axis=0)
 
 
-def decode_attn(q: np.ndarray, T: Tables, zoom_ids: Sequence[Sequence[int]]) -> Tuple[np.ndarray, np.ndarray]:
+def decode_attn(q: np.ndarray, T: Tables, zoom_ids: Sequence[Sequence[int]],
+                heads: Optional[Sequence[int]] = None) -> Tuple[np.ndarray, np.ndarray]:
     """Mixed-resolution attention for every query head of one sequence at one layer.
     ``q`` [H_q, d_h]; ``zoom_ids[g]`` the expanded spans of kv head g.  Returns out [H_q, d_h] and
-    the log-sum-exp [H_q] of each head's softmax."""
+    the log-sum-exp [H_q] of each head's softmax.  ``heads`` restricts the work to a subset of
+    query heads (the other rows stay zero) so that tests can sample large configurations."""
     q = np.asarray(q, dtype=np.float64)
     G = T.group
     out = np.zeros((T.n_q_heads, T.head_dim))
     lse = np.zeros(T.n_q_heads)
-    for h in range(T.n_q_heads):
+    for h in (range(T.n_q_heads) if heads is None else heads):
         g = h // G
         logits, values = mixed_entries(q[h], g, T, zoom_ids[g])
         out[h], lse[h] = softmax_attend(logits, values)

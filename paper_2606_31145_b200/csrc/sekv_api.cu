@@ -1,0 +1,693 @@
+// C-ABI entry points of libsekv: handle, arena layout, build / route / decode orchestration.
+// Every step of the path runs in the CUDA kernels of the other translation units; this file holds
+// argument checking, memory layout, stream/event/graph plumbing and allocation bookkeeping only.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "sekv_internal.cuh"
+
+using namespace sekv;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+
+struct Carver {
+  size_t off = 0;
+  int64_t take(size_t bytes) {
+    off = round_up_sz(off, kAlign);
+    int64_t o = (int64_t)off;
+    off += bytes;
+    return o;
+  }
+};
+
+const char* check_config(const sekv_config* c) {
+  if (!c) return "config is NULL";
+  if (c->n_layers < 1) return "n_layers < 1";
+  if (c->head_dim != SEKV_HEAD_DIM) return "head_dim must be 128";
+  if (c->n_kv_heads < 1 || c->n_q_heads < 1 || c->n_q_heads % c->n_kv_heads) return "n_q_heads must be a multiple of n_kv_heads";
+  if (c->n_q_heads / c->n_kv_heads > SEKV_MAX_GROUP) return "more than 8 query heads per kv head";
+  if (c->route_dim < 8 || c->route_dim > SEKV_MAX_ROUTE_DIM || c->route_dim % 8) return "route_dim must be a multiple of 8 in [8, 64]";
+  if (c->dtype != SEKV_F32 && c->dtype != SEKV_BF16) return "dtype must be SEKV_F32 or SEKV_BF16";
+  if (c->out_dtype != SEKV_F32 && c->out_dtype != SEKV_BF16) return "out_dtype must be SEKV_F32 or SEKV_BF16";
+  if (c->l_min < 1) return "l_min < 1";
+  if (c->r_max < 1 || c->r_max > SEKV_MAX_RANK) return "r_max must be in [1, 64]";
+  if (c->window < 0) return "window < 0";
+  if (c->max_seqs < 1) return "max_seqs < 1";
+  if (c->max_tokens_total < 1) return "max_tokens_total < 1";
+  if (c->max_spans_total < 1 || c->max_full_total < 0) return "bad span / pool capacity";
+  if (c->max_span_len < 1 || c->max_span_len > SEKV_MAX_SPAN_LEN) return "max_span_len must be in [1, 1024]";
+  if (c->k_cap < 0) return "k_cap < 0";
+  if (c->cache_ways < std::max(c->k_cap, 1)) return "cache_ways must be >= max(k_cap, 1)";
+  if (c->cache_ways > 8192) return "cache_ways > 8192";
+  if (c->stage1_ctas < 0 || c->stage1_ctas > 4096) return "stage1_ctas out of range";
+  if (!(c->alpha == c->alpha)) return "alpha is NaN";
+  return nullptr;
+}
+
+void compute_layout(const sekv_config& c, FullLayout* F) {
+  memset(F, 0, sizeof(*F));
+  sekv_layout& L = F->lay;
+  const int64_t es = c.dtype == SEKV_BF16 ? 2 : 4;
+  const int64_t B = c.max_seqs, Hq = c.n_q_heads, Hkv = c.n_kv_heads, NL = c.n_layers;
+  const int64_t mcap = c.max_spans_total, acap = c.max_full_total, rcap = mcap + acap;
+  const int kcap = std::max(c.k_cap, 1);
+  L.esize = es; L.rows_cap = rcap; L.spans_cap = mcap;
+  Carver cv;
+  L.seq_tok_off = cv.take((B + 1) * 8);
+  L.seq_row_off = cv.take((B + 1) * 4);
+  L.seq_span_off = cv.take((B + 1) * 4);
+  L.seq_pool_cnt = cv.take(B * 4);
+  L.span_len = cv.take(mcap * 4);
+  L.span_tok_start = cv.take(mcap * 8);
+  L.ln_len = cv.take(mcap * 4);
+  L.pool_tok = cv.take(std::max<int64_t>(acap, 1) * 8);
+  L.ent_head_stride = rcap * kD * es;
+  L.ent_layer_stride = round_up_sz(Hkv * L.ent_head_stride, kAlign);
+  L.ent_k = cv.take(NL * L.ent_layer_stride);
+  L.ent_v = cv.take(NL * L.ent_layer_stride);
+  L.route_head_stride = mcap * c.route_dim * es;
+  L.route_layer_stride = round_up_sz(Hq * L.route_head_stride, kAlign);
+  L.route = cv.take(NL * L.route_layer_stride);
+  L.w_layer_stride = round_up_sz(Hq * c.route_dim * kD * es, kAlign);
+  L.w = cv.take(NL * L.w_layer_stride);
+  L.dir_layer_stride_elems = Hkv * mcap;
+  L.dir_off = cv.take(NL * L.dir_layer_stride_elems * 8);
+  L.dir_rank = cv.take(NL * L.dir_layer_stride_elems * 4);
+  const int64_t regions = NL * B * Hkv;
+  L.cache_tags = cv.take(regions * c.cache_ways * 4);
+  L.cache_stamps = cv.take(regions * c.cache_ways * 4);
+  BlobDims bd = blob_dims((int)es, c.max_span_len, c.r_max, c.r_max);
+  L.slot_bytes = (int64_t)bd.bytes;
+  L.cache_slots = cv.take((size_t)regions * c.cache_ways * bd.bytes);
+  // workspace
+  F->max_chunks = std::max(c.stage1_ctas, 1024) + (int)(B * Hkv);
+  const int G = c.n_q_heads / c.n_kv_heads;
+  const int P2 = (kcap + kStage2SpansPerCta - 1) / kStage2SpansPerCta;
+  F->off_partials1 = cv.take((size_t)F->max_chunks * G * kPartStride * 4);
+  F->off_partials2 = cv.take((size_t)B * Hkv * P2 * G * kPartStride * 4);
+  F->off_ws_ids = cv.take((size_t)NL * B * Hkv * kcap * 4);
+  F->off_ws_count = cv.take((size_t)NL * B * Hkv * 4);
+  F->off_stats = cv.take(ST_COUNT * 8);
+  F->off_chunks = cv.take((size_t)F->max_chunks * sizeof(Chunk));
+  F->off_bg_chunk = cv.take((size_t)(B * Hkv + 1) * 4);
+  F->mask_words = (int)((std::min<int64_t>(mcap, SEKV_MAX_SPANS_PER_SEQ) + 31) / 32);
+  F->off_zoom_mask = cv.take((size_t)NL * B * Hkv * F->mask_words * 4);
+  F->off_items = cv.take((size_t)NL * B * Hkv * kcap * 4);
+  F->off_item_span = cv.take((size_t)NL * B * Hkv * kcap * 4);
+  F->off_layer_step = cv.take((size_t)NL * 4);
+  F->off_seg_flag = cv.take((size_t)c.max_tokens_total);
+  F->off_seg_flag2 = cv.take((size_t)c.max_tokens_total);
+  F->off_seg_len = cv.take((size_t)c.max_tokens_total * 4);
+  F->off_seg_misc = cv.take((size_t)B * 32);
+  F->off_err_flag = cv.take(16);
+  const int64_t osz = c.out_dtype == SEKV_BF16 ? 2 : 4;
+  F->off_q_stage = cv.take((size_t)NL * B * Hq * kD * es);
+  F->off_out_stage = cv.take((size_t)NL * B * Hq * kD * osz);
+  F->off_lse_stage = cv.take((size_t)NL * B * Hq * 4);
+  F->total = round_up_sz(cv.off, kAlign);
+  L.device_bytes_total = (int64_t)F->total;
+}
+
+sekv_status fail(sekv_handle* h, sekv_status s, const std::string& msg) {
+  if (h) h->err = msg;
+  return s;
+}
+sekv_status cuda_fail(sekv_handle* h, cudaError_t e, const char* where) {
+  char buf[256];
+  snprintf(buf, sizeof(buf), "%s: %s", where, cudaGetErrorString(e));
+  return fail(h, SEKV_CUDA, buf);
+}
+#define CK(h, expr)                                          \
+  do {                                                       \
+    cudaError_t e__ = (expr);                                \
+    if (e__ != cudaSuccess) return cuda_fail(h, e__, #expr); \
+  } while (0)
+
+}  // namespace
+
+namespace sekv {
+
+CsrView csr_view(const sekv_handle* h) {
+  CsrView v;
+  uint8_t* d = h->dev;
+  v.seq_tok_off = (const int64_t*)(d + h->lay.seq_tok_off);
+  v.seq_row_off = (const int32_t*)(d + h->lay.seq_row_off);
+  v.seq_span_off = (const int32_t*)(d + h->lay.seq_span_off);
+  v.seq_pool_cnt = (const int32_t*)(d + h->lay.seq_pool_cnt);
+  v.span_len = (const int32_t*)(d + h->lay.span_len);
+  v.span_tok_start = (const int64_t*)(d + h->lay.span_tok_start);
+  v.ln_len = (const float*)(d + h->lay.ln_len);
+  v.pool_tok = (const int64_t*)(d + h->lay.pool_tok);
+  return v;
+}
+
+LayerView layer_view(const sekv_handle* h, int l) {
+  LayerView v;
+  uint8_t* d = h->dev;
+  const sekv_layout& L = h->lay;
+  const sekv_config& c = h->cfg;
+  const int64_t B = c.max_seqs, Hkv = c.n_kv_heads;
+  const int kcap = std::max(c.k_cap, 1);
+  v.ent_k = d + L.ent_k + (int64_t)l * L.ent_layer_stride;
+  v.ent_v = d + L.ent_v + (int64_t)l * L.ent_layer_stride;
+  v.route = d + L.route + (int64_t)l * L.route_layer_stride;
+  v.W = d + L.w + (int64_t)l * L.w_layer_stride;
+  v.dir_off = (const int64_t*)(d + L.dir_off) + (int64_t)l * L.dir_layer_stride_elems;
+  v.dir_rank = (const int32_t*)(d + L.dir_rank) + (int64_t)l * L.dir_layer_stride_elems;
+  const int64_t region0 = (int64_t)l * B * Hkv;
+  v.tags = (int32_t*)(d + L.cache_tags) + region0 * c.cache_ways;
+  v.stamps = (uint32_t*)(d + L.cache_stamps) + region0 * c.cache_ways;
+  v.slots = d + L.cache_slots + (size_t)region0 * c.cache_ways * L.slot_bytes;
+  v.layer_step = (uint32_t*)(d + h->F.off_layer_step) + l;
+  v.zoom_mask = (uint32_t*)(d + h->F.off_zoom_mask) + region0 * h->mask_words;
+  v.items = (uint32_t*)(d + h->F.off_items) + region0 * kcap;
+  v.item_span = (int32_t*)(d + h->F.off_item_span) + region0 * kcap;
+  return v;
+}
+
+}  // namespace sekv
+
+extern "C" {
+
+const char* sekv_version(void) { return "sekv-b200 0.1 (sm_100a)"; }
+
+const char* sekv_status_string(sekv_status s) {
+  switch (s) {
+    case SEKV_OK: return "SEKV_OK";
+    case SEKV_INVALID_ARG: return "SEKV_INVALID_ARG";
+    case SEKV_UNSUPPORTED: return "SEKV_UNSUPPORTED";
+    case SEKV_OOM_DEVICE: return "SEKV_OOM_DEVICE";
+    case SEKV_OOM_HOST: return "SEKV_OOM_HOST";
+    case SEKV_CUDA: return "SEKV_CUDA";
+    case SEKV_STATE: return "SEKV_STATE";
+  }
+  return "SEKV_?";
+}
+
+sekv_status sekv_device_arena_bytes(const sekv_config* cfg, size_t* device_bytes, size_t* slot_bytes) {
+  if (check_config(cfg)) return SEKV_INVALID_ARG;
+  FullLayout F;
+  compute_layout(*cfg, &F);
+  if (device_bytes) *device_bytes = F.total;
+  if (slot_bytes) *slot_bytes = (size_t)F.lay.slot_bytes;
+  return SEKV_OK;
+}
+
+size_t sekv_blob_bytes(int32_t dtype, int32_t span_len, int32_t rank_k, int32_t rank_v) {
+  return blob_dims(dtype == SEKV_BF16 ? 2 : 4, span_len, rank_k, rank_v).bytes;
+}
+
+sekv_status sekv_create(const sekv_config* cfg, void* device_arena, size_t device_bytes, void* host_arena,
+                        size_t host_bytes, sekv_handle** out) {
+  if (!out) return SEKV_INVALID_ARG;
+  *out = nullptr;
+  if (check_config(cfg)) return SEKV_INVALID_ARG;
+  if (!device_arena || ((uintptr_t)device_arena % kAlign)) return SEKV_INVALID_ARG;
+  if (!host_arena || ((uintptr_t)host_arena % 128)) return SEKV_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return SEKV_CUDA; }
+  sekv_handle* h = new (std::nothrow) sekv_handle();
+  if (!h) return SEKV_OOM_HOST;
+  h->registered_host = false;
+  h->cfg = *cfg;
+  h->G = cfg->n_q_heads / cfg->n_kv_heads;
+  h->esize = cfg->dtype == SEKV_BF16 ? 2 : 4;
+  compute_layout(*cfg, &h->F);
+  h->lay = h->F.lay;
+  if (device_bytes < h->F.total) { delete h; return SEKV_OOM_DEVICE; }
+  h->dev = (uint8_t*)device_arena; h->dev_bytes = device_bytes;
+  h->host = (uint8_t*)host_arena; h->host_bytes = host_bytes;
+  const FullLayout& F = h->F;
+  h->mask_words = F.mask_words;
+  h->main = (cudaStream_t)cfg->main_stream;
+  h->side = (cudaStream_t)cfg->side_stream;
+  h->own_side = false;
+  cudaError_t e;
+  void* hd = nullptr;
+  e = cudaHostGetDevicePointer(&hd, host_arena, 0);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    e = cudaHostRegister(host_arena, host_bytes, cudaHostRegisterMapped | cudaHostRegisterPortable);
+    if (e == cudaSuccess) { h->registered_host = true; e = cudaHostGetDevicePointer(&hd, host_arena, 0); }
+  }
+  if (e != cudaSuccess) { cudaGetLastError(); if (h->registered_host) cudaHostUnregister(host_arena); delete h; return SEKV_CUDA; }
+  h->host_dev = (uint8_t*)hd;
+  if (!h->side) {
+    if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); delete h; return SEKV_CUDA; }
+    h->own_side = true;
+  }
+  cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  h->launches = 0;
+  *out = h;
+  sekv_status s = sekv_reset(h);
+  if (s != SEKV_OK) { sekv_destroy(h); *out = nullptr; return s; }
+  return SEKV_OK;
+}
+
+void sekv_destroy(sekv_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->main);
+  cudaStreamSynchronize(h->side);
+  for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+  if (h->own_side) cudaStreamDestroy(h->side);
+  cudaEventDestroy(h->ev_fork);
+  cudaEventDestroy(h->ev_join);
+  if (h->registered_host) cudaHostUnregister(h->host);
+  delete h;
+}
+
+const char* sekv_last_error(const sekv_handle* h) { return h ? h->err.c_str() : "null handle"; }
+
+sekv_status sekv_reset(sekv_handle* h) {
+  if (!h) return SEKV_INVALID_ARG;
+  const FullLayout& F = h->F;
+  const sekv_config& c = h->cfg;
+  CK(h, cudaStreamSynchronize(h->main));
+  CK(h, cudaStreamSynchronize(h->side));
+  for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+  h->graphs.clear();
+  const int64_t regions = (int64_t)c.n_layers * c.max_seqs * c.n_kv_heads;
+  CK(h, cudaMemsetAsync(h->dev + h->lay.cache_tags, 0xFF, regions * c.cache_ways * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + h->lay.cache_stamps, 0, regions * c.cache_ways * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_layer_step, 0, (size_t)c.n_layers * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_stats, 0, ST_COUNT * 8, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_err_flag, 0, 16, h->main));
+  CK(h, cudaStreamSynchronize(h->main));
+  h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
+  h->span_len_host.clear();
+  h->m_tot = h->A_tot = h->max_m = 0;
+  h->layer_built.assign(c.n_layers, 0);
+  h->host_used = 0;
+  h->n_chunks = 0; h->parts1_max = 0; h->sort_n = 0;
+  h->P2 = (std::max(c.k_cap, 1) + kStage2SpansPerCta - 1) / kStage2SpansPerCta;
+  h->parts_per_head = 0;
+  h->err.clear();
+  return SEKV_OK;
+}
+
+sekv_status sekv_cache_flush(sekv_handle* h) {
+  if (!h) return SEKV_INVALID_ARG;
+  const sekv_config& c = h->cfg;
+  const int64_t regions = (int64_t)c.n_layers * c.max_seqs * c.n_kv_heads;
+  CK(h, cudaStreamSynchronize(h->side));
+  CK(h, cudaMemsetAsync(h->dev + h->lay.cache_tags, 0xFF, regions * c.cache_ways * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + h->lay.cache_stamps, 0, regions * c.cache_ways * 4, h->main));
+  return SEKV_OK;
+}
+
+// ---- build -------------------------------------------------------------------------------------------
+static sekv_status make_schedule(sekv_handle* h) {
+  // Static stage-1 schedule: entry rows of every (sequence, kv head) cut into near-equal chunks so
+  // that the grid is ~ stage1_ctas CTAs of equal work (ragged contexts).
+  const FullLayout& F = h->F;
+  const sekv_config& c = h->cfg;
+  const int B = h->n_seqs, Hkv = c.n_kv_heads;
+  int target_ctas = c.stage1_ctas > 0 ? c.stage1_ctas : h->num_sms * 4;
+  long total_tiles = 0;
+  std::vector<int> tiles(B);
+  for (int b = 0; b < B; ++b) {
+    tiles[b] = (h->A_b[b] + h->m_b[b] + kTile - 1) / kTile;
+    total_tiles += (long)tiles[b] * Hkv;
+  }
+  std::vector<Chunk> chunks;
+  std::vector<int32_t> bg_begin(B * Hkv + 1, 0);
+  int parts1_max = 0;
+  for (int b = 0; b < B; ++b) {
+    int rows = h->A_b[b] + h->m_b[b];
+    int n = 0;
+    if (rows > 0) {
+      double share = total_tiles > 0 ? (double)tiles[b] * target_ctas / (double)total_tiles : 1.0;
+      n = std::max(1, (int)std::floor(share + 0.5));
+      n = std::min(n, tiles[b]);
+    }
+    for (int g = 0; g < Hkv; ++g) {
+      bg_begin[b * Hkv + g] = (int32_t)chunks.size();
+      if (n == 0) continue;
+      int per = (tiles[b] + n - 1) / n;
+      int part = 0;
+      for (int t0 = 0; t0 < tiles[b]; t0 += per, ++part) {
+        Chunk ck;
+        ck.bg = b * Hkv + g;
+        ck.row_begin = t0 * kTile;
+        ck.row_end = std::min(rows, (t0 + per) * kTile);
+        ck.part = part;
+        chunks.push_back(ck);
+      }
+      parts1_max = std::max(parts1_max, part);
+    }
+  }
+  bg_begin[B * Hkv] = (int32_t)chunks.size();
+  if ((int)chunks.size() > F.max_chunks) return fail(h, SEKV_UNSUPPORTED, "stage-1 schedule exceeds chunk capacity");
+  h->n_chunks = (int)chunks.size();
+  h->parts1_max = parts1_max;
+  h->parts_per_head = parts1_max + h->P2;
+  if (!chunks.empty())
+    CK(h, cudaMemcpyAsync(h->dev + F.off_chunks, chunks.data(), chunks.size() * sizeof(Chunk), cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_chunk, bg_begin.data(), bg_begin.size() * 4, cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaStreamSynchronize(h->main));
+  int sn = 32;
+  while (sn < h->max_m) sn <<= 1;
+  h->sort_n = sn;
+  return SEKV_OK;
+}
+
+static sekv_status ensure_segmented(sekv_handle* h, int n_seqs, const int64_t* seq_tok_off, const float* H) {
+  const sekv_config& c = h->cfg;
+  if (n_seqs < 1 || n_seqs > c.max_seqs) return fail(h, SEKV_INVALID_ARG, "n_seqs out of range");
+  if (!seq_tok_off) return fail(h, SEKV_INVALID_ARG, "seq_tok_off is NULL");
+  if (seq_tok_off[0] != 0) return fail(h, SEKV_INVALID_ARG, "seq_tok_off[0] != 0");
+  for (int b = 0; b < n_seqs; ++b)
+    if (seq_tok_off[b + 1] <= seq_tok_off[b]) return fail(h, SEKV_INVALID_ARG, "empty or negative-length sequence");
+  if (seq_tok_off[n_seqs] > c.max_tokens_total) return fail(h, SEKV_OOM_DEVICE, "sum of tokens exceeds max_tokens_total");
+  if (h->segmented) {
+    if (n_seqs != h->n_seqs) return fail(h, SEKV_STATE, "batch size differs from the segmented batch");
+    for (int b = 0; b <= n_seqs; ++b)
+      if (seq_tok_off[b] != h->tok_off[b]) return fail(h, SEKV_STATE, "token offsets differ from the segmented batch");
+    return SEKV_OK;
+  }
+  if (!H) return fail(h, SEKV_INVALID_ARG, "H is NULL on the first build call");
+  std::vector<int> m(n_seqs), a(n_seqs);
+  std::string why;
+  h->n_seqs = n_seqs;
+  cudaError_t e = launch_segment(h, H, n_seqs, seq_tok_off, m.data(), a.data(), &why);
+  if (e != cudaSuccess) { h->n_seqs = 0; return cuda_fail(h, e, "segmentation"); }
+  if (!why.empty()) { h->n_seqs = 0; return fail(h, why.find("capacity") != std::string::npos ? SEKV_OOM_DEVICE : SEKV_UNSUPPORTED, why); }
+  h->m_b = m; h->A_b = a;
+  h->tok_off.assign(seq_tok_off, seq_tok_off + n_seqs + 1);
+  h->m_tot = 0; h->A_tot = 0; h->max_m = 0;
+  for (int b = 0; b < n_seqs; ++b) { h->m_tot += m[b]; h->A_tot += a[b]; h->max_m = std::max(h->max_m, m[b]); }
+  h->segmented = true;
+  return make_schedule(h);
+}
+
+static sekv_status assign_blobs(sekv_handle* h, int layer, const std::vector<int32_t>& rk, const std::vector<int32_t>& rv) {
+  // rk, rv: [H_kv][m_tot] retained ranks (host copies).  Bump-allocates the host arena.
+  const sekv_config& c = h->cfg;
+  const int Hkv = c.n_kv_heads, m = h->m_tot;
+  std::vector<int64_t> off((size_t)Hkv * h->lay.spans_cap, 0);
+  std::vector<int32_t> rank((size_t)Hkv * h->lay.spans_cap, 0);
+  size_t used = round_up_sz(h->host_used, 128);
+  for (int g = 0; g < Hkv; ++g)
+    for (int s = 0; s < m; ++s) {
+      int len = h->span_len_host[s];
+      int a = rk[(size_t)g * m + s], b = rv[(size_t)g * m + s];
+      if (a < 0 || b < 0 || a > c.r_max || b > c.r_max || a > len || b > len)
+        return fail(h, SEKV_INVALID_ARG, "retained rank out of range (must be <= min(r_max, |S|))");
+      BlobDims bd = blob_dims(h->esize, len, a, b);
+      off[(size_t)g * h->lay.spans_cap + s] = (int64_t)used;
+      rank[(size_t)g * h->lay.spans_cap + s] = a | (b << 8);
+      used += bd.bytes;
+    }
+  if (used > h->host_bytes) return fail(h, SEKV_OOM_HOST, "pinned host arena too small for the factor store");
+  LayerView lv = layer_view(h, layer);
+  CK(h, cudaMemcpyAsync((void*)lv.dir_off, off.data(), off.size() * 8, cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaMemcpyAsync((void*)lv.dir_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaStreamSynchronize(h->main));
+  h->host_used = used;
+  return SEKV_OK;
+}
+
+static void report_counts(sekv_handle* h, int32_t* spans_per_seq, int32_t* pool_per_seq) {
+  for (int b = 0; b < h->n_seqs; ++b) {
+    if (spans_per_seq) spans_per_seq[b] = h->m_b[b];
+    if (pool_per_seq) pool_per_seq[b] = h->A_b[b];
+  }
+}
+
+sekv_status sekv_build_spans_prefactored(sekv_handle* h, int32_t layer, int32_t n_seqs, const int64_t* seq_tok_off,
+                                         const float* H, const sekv_factors* f, const void* W,
+                                         int32_t* spans_per_seq, int32_t* pool_per_seq) {
+  if (!h) return SEKV_INVALID_ARG;
+  const sekv_config& c = h->cfg;
+  if (layer < 0 || layer >= c.n_layers) return fail(h, SEKV_INVALID_ARG, "layer out of range");
+  if (!f || !W) return fail(h, SEKV_INVALID_ARG, "factors or W is NULL");
+  if (f->rank_in < 1 || f->rank_in > SEKV_MAX_RANK) return fail(h, SEKV_INVALID_ARG, "rank_in out of range");
+  if (!f->tokUK || !f->SK || !f->VtK || !f->tokUV || !f->SV || !f->VtV) return fail(h, SEKV_INVALID_ARG, "NULL factor array");
+  if (!H) return fail(h, SEKV_INVALID_ARG, "H is NULL (the summaries need the surprisal weights)");
+  sekv_status s = ensure_segmented(h, n_seqs, seq_tok_off, H);
+  if (s != SEKV_OK) return s;
+  if (f->m_tot != h->m_tot || f->a_tot != h->A_tot) {
+    char buf[160];
+    snprintf(buf, sizeof(buf), "segmentation found m_tot=%d A_tot=%d but the factors were laid out for m_tot=%d A_tot=%d",
+             h->m_tot, h->A_tot, f->m_tot, f->a_tot);
+    return fail(h, SEKV_STATE, buf);
+  }
+  if (h->A_tot > 0 && (!f->Kfull || !f->Vfull)) return fail(h, SEKV_INVALID_ARG, "Kfull/Vfull is NULL");
+  const int Hkv = c.n_kv_heads, m = h->m_tot;
+  std::vector<int32_t> rk((size_t)Hkv * m), rv((size_t)Hkv * m);
+  if (f->rank_k) CK(h, cudaMemcpy(rk.data(), f->rank_k, rk.size() * 4, cudaMemcpyDeviceToHost));
+  if (f->rank_v) CK(h, cudaMemcpy(rv.data(), f->rank_v, rv.size() * 4, cudaMemcpyDeviceToHost));
+  for (int g = 0; g < Hkv; ++g)
+    for (int sidx = 0; sidx < m; ++sidx) {
+      int cap = std::min({(int)f->rank_in, h->span_len_host[sidx], c.r_max});
+      if (!f->rank_k) rk[(size_t)g * m + sidx] = cap;
+      if (!f->rank_v) rv[(size_t)g * m + sidx] = cap;
+      if (rk[(size_t)g * m + sidx] > f->rank_in || rv[(size_t)g * m + sidx] > f->rank_in)
+        return fail(h, SEKV_INVALID_ARG, "retained rank exceeds rank_in");
+    }
+  s = assign_blobs(h, layer, rk, rv);
+  if (s != SEKV_OK) return s;
+  cudaError_t e = launch_build_prefactored(h, layer, H, f, W);
+  if (e != cudaSuccess) return cuda_fail(h, e, "build (prefactored)");
+  CK(h, cudaStreamSynchronize(h->main));
+  h->layer_built[layer] = 1;
+  report_counts(h, spans_per_seq, pool_per_seq);
+  return SEKV_OK;
+}
+
+sekv_status sekv_build_spans(sekv_handle* h, int32_t layer, int32_t n_seqs, const int64_t* seq_tok_off,
+                             const float* H, const void* K, const void* V, const void* W, int32_t rank_cap,
+                             int32_t* spans_per_seq, int32_t* pool_per_seq) {
+  if (!h) return SEKV_INVALID_ARG;
+  const sekv_config& c = h->cfg;
+  if (layer < 0 || layer >= c.n_layers) return fail(h, SEKV_INVALID_ARG, "layer out of range");
+  if (!K || !V || !W) return fail(h, SEKV_INVALID_ARG, "K, V or W is NULL");
+  if (!H) return fail(h, SEKV_INVALID_ARG, "H is NULL (the summaries need the surprisal weights)");
+  if (rank_cap < 0 || rank_cap > c.r_max) return fail(h, SEKV_INVALID_ARG, "rank_cap out of range");
+  if (rank_cap == 0) rank_cap = c.r_max;
+  sekv_status s = ensure_segmented(h, n_seqs, seq_tok_off, H);
+  if (s != SEKV_OK) return s;
+  const int Hkv = c.n_kv_heads, m = h->m_tot;
+  std::vector<int32_t> rk((size_t)Hkv * m), rv;
+  for (int g = 0; g < Hkv; ++g)
+    for (int sidx = 0; sidx < m; ++sidx)
+      rk[(size_t)g * m + sidx] = std::min({rank_cap, h->span_len_host[sidx], (int)kD});   // Eq. 6: R = min(|S|, d_h, R_max)
+  rv = rk;
+  s = assign_blobs(h, layer, rk, rv);
+  if (s != SEKV_OK) return s;
+  std::string why;
+  cudaError_t e = launch_build_dense(h, layer, H, K, V, W, rank_cap, &why);
+  if (e != cudaSuccess) return cuda_fail(h, e, "build (dense)");
+  if (!why.empty()) return fail(h, SEKV_UNSUPPORTED, why);
+  CK(h, cudaStreamSynchronize(h->main));
+  h->layer_built[layer] = 1;
+  report_counts(h, spans_per_seq, pool_per_seq);
+  return SEKV_OK;
+}
+
+// ---- decode --------------------------------------------------------------------------------------------
+static sekv_status check_ready(sekv_handle* h, int layer) {
+  if (!h->segmented) return fail(h, SEKV_STATE, "no sequences built");
+  if (layer < 0 || layer >= h->cfg.n_layers) return fail(h, SEKV_INVALID_ARG, "layer out of range");
+  if (!h->layer_built[layer]) return fail(h, SEKV_STATE, "layer not built");
+  return SEKV_OK;
+}
+
+static sekv_status check_k(sekv_handle* h, int k) {
+  if (k > h->cfg.k_cap) return fail(h, SEKV_INVALID_ARG, "k exceeds k_cap");
+  if (k < 0 && h->max_m > h->cfg.k_cap) return fail(h, SEKV_INVALID_ARG, "k < 0 (all spans) needs k_cap >= spans per sequence");
+  return SEKV_OK;
+}
+
+sekv_status sekv_route(sekv_handle* h, int32_t layer, const void* q, const float* tau, int32_t k, float* logits,
+                       float* alpha_tilde, int32_t* ids, int32_t* count) {
+  if (!h) return SEKV_INVALID_ARG;
+  sekv_status s = check_ready(h, layer);
+  if (s != SEKV_OK) return s;
+  if (!q || !ids || !count) return fail(h, SEKV_INVALID_ARG, "q, ids or count is NULL");
+  if ((s = check_k(h, k)) != SEKV_OK) return s;
+  cudaError_t e = launch_route(h, layer, q, tau, k, logits, alpha_tilde, ids, count, h->main);
+  if (e != cudaSuccess) return cuda_fail(h, e, "route");
+  return SEKV_OK;
+}
+
+static cudaError_t decode_layer(sekv_handle* h, int layer, const void* q, const int32_t* ids, const int32_t* count,
+                                void* out, float* lse) {
+  cudaError_t e;
+  if ((e = launch_plan(h, layer, ids, count, h->main)) != cudaSuccess) return e;
+  if (h->cfg.k_cap > 0) {
+    if ((e = cudaEventRecord(h->ev_fork, h->main)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(h->side, h->ev_fork, 0)) != cudaSuccess) return e;
+    if ((e = launch_fetch(h, layer, count, h->side)) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(h->ev_join, h->side)) != cudaSuccess) return e;
+  }
+  if ((e = launch_stage1(h, layer, q, h->main)) != cudaSuccess) return e;
+  if (h->cfg.k_cap > 0) {
+    if ((e = cudaStreamWaitEvent(h->main, h->ev_join, 0)) != cudaSuccess) return e;
+    if ((e = launch_stage2(h, layer, q, count, h->main)) != cudaSuccess) return e;
+  }
+  return launch_combine(h, layer, out, lse, h->main);
+}
+
+sekv_status sekv_decode_attn(sekv_handle* h, int32_t layer, const void* q, const int32_t* ids, const int32_t* count,
+                             void* out, float* lse) {
+  if (!h) return SEKV_INVALID_ARG;
+  sekv_status s = check_ready(h, layer);
+  if (s != SEKV_OK) return s;
+  if (!q || !out) return fail(h, SEKV_INVALID_ARG, "q or out is NULL");
+  if (h->cfg.k_cap > 0 && (!ids || !count)) return fail(h, SEKV_INVALID_ARG, "ids or count is NULL");
+  cudaError_t e = decode_layer(h, layer, q, ids, count, out, lse);
+  if (e != cudaSuccess) return cuda_fail(h, e, "decode_attn");
+  return SEKV_OK;
+}
+
+static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau, int k, void* out, float* lse) {
+  const sekv_config& c = h->cfg;
+  const int B = h->n_seqs;
+  const size_t qstride = (size_t)B * c.n_q_heads * kD * h->esize;
+  const size_t ostride = (size_t)B * c.n_q_heads * kD * (c.out_dtype == SEKV_BF16 ? 2 : 4);
+  const int kcap = std::max(c.k_cap, 1);
+  for (int l = 0; l < c.n_layers; ++l) {
+    const uint8_t* ql = (const uint8_t*)q + l * qstride;
+    int32_t* ids = (int32_t*)(h->dev + h->F.off_ws_ids) + (size_t)l * c.max_seqs * c.n_kv_heads * kcap;
+    int32_t* cnt = (int32_t*)(h->dev + h->F.off_ws_count) + (size_t)l * c.max_seqs * c.n_kv_heads;
+    cudaError_t e;
+    if (c.k_cap > 0) {
+      e = launch_route(h, l, ql, tau ? tau + (size_t)l * c.n_q_heads : nullptr, k, nullptr, nullptr, ids, cnt, h->main);
+      if (e != cudaSuccess) return e;
+    }
+    e = decode_layer(h, l, ql, ids, cnt, (uint8_t*)out + l * ostride, lse ? lse + (size_t)l * B * c.n_q_heads : nullptr);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out, float* lse) {
+  if (!h) return SEKV_INVALID_ARG;
+  if (!h->segmented) return fail(h, SEKV_STATE, "no sequences built");
+  for (int l = 0; l < h->cfg.n_layers; ++l)
+    if (!h->layer_built[l]) return fail(h, SEKV_STATE, "not every layer is built");
+  if (!q || !out) return fail(h, SEKV_INVALID_ARG, "q or out is NULL");
+  sekv_status s = check_k(h, k);
+  if (s != SEKV_OK) return s;
+  if (!h->cfg.use_graph) {
+    cudaError_t e = enqueue_step(h, q, tau, k, out, lse);
+    if (e != cudaSuccess) return cuda_fail(h, e, "decode_step");
+    return SEKV_OK;
+  }
+  for (auto& g : h->graphs)
+    if (g.q == q && g.tau == tau && g.k == k && g.out == out && g.lse == lse) {
+      CK(h, cudaGraphLaunch(g.exec, h->main));
+      h->launches += g.nodes;
+      return SEKV_OK;
+    }
+  // capture once for this argument tuple
+  uint64_t before = h->launches;
+  CK(h, cudaStreamBeginCapture(h->main, cudaStreamCaptureModeRelaxed));
+  cudaError_t e = enqueue_step(h, q, tau, k, out, lse);
+  cudaGraph_t graph = nullptr;
+  cudaError_t e2 = cudaStreamEndCapture(h->main, &graph);
+  uint64_t nodes = h->launches - before;
+  h->launches = before;
+  if (e != cudaSuccess || e2 != cudaSuccess) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    return cuda_fail(h, e != cudaSuccess ? e : e2, "decode_step graph capture");
+  }
+  GraphEntry ge{q, tau, k, out, lse, nullptr, nodes};
+  cudaError_t e3 = cudaGraphInstantiate(&ge.exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e3 != cudaSuccess) return cuda_fail(h, e3, "cudaGraphInstantiate");
+  if (h->graphs.size() >= 64) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
+  h->graphs.push_back(ge);
+  CK(h, cudaGraphLaunch(ge.exec, h->main));
+  h->launches += nodes;
+  return SEKV_OK;
+}
+
+sekv_status sekv_decode_step_host(sekv_handle* h, const void* q_host, const float* tau, int32_t k, void* out_host,
+                                  float* lse_host) {
+  if (!h) return SEKV_INVALID_ARG;
+  if (!q_host || !out_host) return fail(h, SEKV_INVALID_ARG, "q_host or out_host is NULL");
+  if (!h->segmented) return fail(h, SEKV_STATE, "no sequences built");
+  const sekv_config& c = h->cfg;
+  const size_t n = (size_t)c.n_layers * h->n_seqs * c.n_q_heads;
+  void* qd = h->dev + h->F.off_q_stage;
+  void* od = h->dev + h->F.off_out_stage;
+  float* ld = (float*)(h->dev + h->F.off_lse_stage);
+  CK(h, cudaMemcpyAsync(qd, q_host, n * kD * h->esize, cudaMemcpyHostToDevice, h->main));
+  sekv_status s = sekv_decode_step(h, qd, tau, k, od, lse_host ? ld : nullptr);
+  if (s != SEKV_OK) return s;
+  CK(h, cudaMemcpyAsync(out_host, od, n * kD * (c.out_dtype == SEKV_BF16 ? 2 : 4), cudaMemcpyDeviceToHost, h->main));
+  if (lse_host) CK(h, cudaMemcpyAsync(lse_host, ld, n * 4, cudaMemcpyDeviceToHost, h->main));
+  CK(h, cudaStreamSynchronize(h->main));
+  return SEKV_OK;
+}
+
+// ---- introspection ----------------------------------------------------------------------------------------
+sekv_status sekv_get_layout(const sekv_handle* h, sekv_layout* out) {
+  if (!h || !out) return SEKV_INVALID_ARG;
+  *out = h->lay;
+  out->host_bytes_used = (int64_t)h->host_used;
+  return SEKV_OK;
+}
+
+sekv_status sekv_get_stats(sekv_handle* h, sekv_stats* out) {
+  if (!h || !out) return SEKV_INVALID_ARG;
+  CK(h, cudaStreamSynchronize(h->main));
+  CK(h, cudaStreamSynchronize(h->side));
+  uint64_t v[ST_COUNT];
+  CK(h, cudaMemcpy(v, h->dev + h->F.off_stats, sizeof(v), cudaMemcpyDeviceToHost));
+  out->layer_steps = v[ST_LAYER_STEPS];
+  out->zoomed_spans = v[ST_ZOOMED];
+  out->cache_hits = v[ST_HITS];
+  out->cache_misses = v[ST_MISSES];
+  out->h2d_bytes = v[ST_H2D];
+  out->factor_bytes_algo = v[ST_FACTOR_ALGO];
+  out->coarse_rows_skipped = v[ST_SKIPPED];
+  out->kernel_launches = h->launches;
+  return SEKV_OK;
+}
+
+sekv_status sekv_reset_stats(sekv_handle* h) {
+  if (!h) return SEKV_INVALID_ARG;
+  CK(h, cudaMemsetAsync(h->dev + h->F.off_stats, 0, ST_COUNT * 8, h->main));
+  h->launches = 0;
+  return SEKV_OK;
+}
+
+sekv_status sekv_static_bytes_per_layer(const sekv_handle* h, uint64_t* bytes) {
+  if (!h || !bytes) return SEKV_INVALID_ARG;
+  const sekv_config& c = h->cfg;
+  const uint64_t b = h->esize, bo = c.out_dtype == SEKV_BF16 ? 2 : 4;
+  uint64_t t = (uint64_t)c.n_q_heads * c.route_dim * kD * b;   // W, once per layer
+  for (int s = 0; s < h->n_seqs; ++s) {
+    const uint64_t m = h->m_b[s], a = h->A_b[s];
+    t += (uint64_t)c.n_q_heads * m * c.route_dim * b + 4 * m;   // routing summaries + ln|S|
+    t += 2ull * c.n_kv_heads * a * kD * b;                      // pool K and V
+    t += 2ull * c.n_kv_heads * m * kD * b;                      // coarse means (all; skipped rows subtracted via stats)
+    t += (uint64_t)c.n_q_heads * kD * (b + bo);                 // q and out
+  }
+  *bytes = t;
+  return SEKV_OK;
+}
+
+sekv_status sekv_get_schedule(const sekv_handle* h, int32_t* stage1_ctas, int32_t* parts_per_head) {
+  if (!h) return SEKV_INVALID_ARG;
+  if (stage1_ctas) *stage1_ctas = h->n_chunks;
+  if (parts_per_head) *parts_per_head = h->parts_per_head;
+  return SEKV_OK;
+}
+
+}  // extern "C"
+

@@ -1,0 +1,214 @@
+// Internal declarations shared by the translation units of libsekv (not part of the ABI).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "sekv.h"
+
+namespace sekv {
+
+constexpr int kD = SEKV_HEAD_DIM;   // d_h
+constexpr int kRankPad = 8;         // ranks padded to a multiple of this in a blob
+constexpr int kLenPad = 16;         // |S| padded to a multiple of this in a blob
+constexpr int kTile = 16;           // stage-1 schedules entry rows in tiles of 16
+constexpr int kPartStride = kD + 4; // floats per partial: m2, l, pad, pad, o[128]
+constexpr int kStage2SpansPerCta = 4;
+
+__host__ __device__ inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+__host__ __device__ inline size_t round_up_sz(size_t x, size_t m) { return (x + m - 1) / m * m; }
+
+// ---- factor blob layout ------------------------------------------------
+// [sigma_K f32 rkp][sigma_V f32 rvp][VtK st rkp x 128][VV st 128 x rvp][UK st lenp x rkp][UVt st rvp x lenp]
+// Each operand is stored with its contraction index contiguous.
+struct BlobDims {
+  int len, lenp, rk, rv, rkp, rvp;
+  size_t off_sk, off_sv, off_vtk, off_vv, off_uk, off_uvt, bytes;
+};
+__host__ __device__ inline BlobDims blob_dims(int esize, int len, int rk, int rv) {
+  BlobDims b;
+  b.len = len; b.rk = rk; b.rv = rv;
+  b.lenp = round_up(len, kLenPad);
+  b.rkp = round_up(rk > 0 ? rk : 1, kRankPad);
+  b.rvp = round_up(rv > 0 ? rv : 1, kRankPad);
+  size_t o = 0;
+  b.off_sk = o;  o += (size_t)b.rkp * 4;
+  b.off_sv = o;  o += (size_t)b.rvp * 4;
+  b.off_vtk = o; o += (size_t)b.rkp * kD * esize;
+  b.off_vv = o;  o += (size_t)kD * b.rvp * esize;
+  b.off_uk = o;  o += (size_t)b.lenp * b.rkp * esize;
+  b.off_uvt = o; o += (size_t)b.rvp * b.lenp * esize;
+  b.bytes = round_up_sz(o, 128);
+  return b;
+}
+
+// ---- device views ------------------------------------------------------------------------------
+struct CsrView {
+  const int64_t* seq_tok_off;
+  const int32_t* seq_row_off;
+  const int32_t* seq_span_off;
+  const int32_t* seq_pool_cnt;
+  const int32_t* span_len;
+  const int64_t* span_tok_start;
+  const float* ln_len;
+  const int64_t* pool_tok;
+};
+
+struct LayerView {
+  const void* ent_k;       // [H_kv][rows_cap][128]
+  const void* ent_v;
+  const void* route;       // [H][spans_cap][d']
+  const void* W;           // [H][d'][128]
+  const int64_t* dir_off;  // [H_kv][spans_cap]
+  const int32_t* dir_rank;
+  int32_t* tags;           // [B][H_kv][ways]
+  uint32_t* stamps;
+  uint8_t* slots;          // [B][H_kv][ways][slot_bytes]
+  uint32_t* layer_step;    // [1]
+  uint32_t* zoom_mask;     // [B][H_kv][mask_words]
+  uint32_t* items;         // [B][H_kv][k_cap]  way | miss << 31, valid for j < count
+  int32_t* item_span;      // [B][H_kv][k_cap]  local span id (deduplicated; -1 = dropped)
+};
+
+struct Dims {
+  int L, Hq, Hkv, G, dp, B, k_cap, ways, mask_words;
+  int rows_cap, spans_cap;
+  int esize;
+  int64_t slot_bytes;
+  int parts1_max, P2, parts_per_head;
+};
+
+struct Chunk {  // one stage-1 work item
+  int32_t bg;         // b * H_kv + g
+  int32_t row_begin;  // local entry row range within the sequence
+  int32_t row_end;
+  int32_t part;       // partial slot within the head
+};
+
+enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_COUNT = 8 };
+
+// ---- storage-type helpers ------------------------------------------------------------------------
+template <typename ST> struct StTraits;
+template <> struct StTraits<float> {
+  static __device__ __forceinline__ float ld(const float* p) { return *p; }
+  static __device__ __forceinline__ void st(float* p, float v) { *p = v; }
+};
+template <> struct StTraits<__nv_bfloat16> {
+  static __device__ __forceinline__ float ld(const __nv_bfloat16* p) { return __bfloat162float(*p); }
+  static __device__ __forceinline__ void st(__nv_bfloat16* p, float v) { *p = __float2bfloat16_rn(v); }
+};
+
+// load 4 consecutive storage elements as floats (16-byte aligned for f32, 8-byte for bf16)
+__device__ __forceinline__ void ld4(const float* p, float (&o)[4]) {
+  float4 v = *reinterpret_cast<const float4*>(p);
+  o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+}
+__device__ __forceinline__ void ld4(const __nv_bfloat16* p, float (&o)[4]) {
+  uint2 v = *reinterpret_cast<const uint2*>(p);
+  o[0] = __uint_as_float(v.x << 16); o[1] = __uint_as_float(v.x & 0xffff0000u);
+  o[2] = __uint_as_float(v.y << 16); o[3] = __uint_as_float(v.y & 0xffff0000u);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// exp2 that maps (-inf) - (-inf) safely: callers guard m == -inf themselves
+__device__ __forceinline__ float fast_exp2(float x) { return exp2f(x); }
+
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+}  // namespace sekv
+
+// ---- host handle -----------------------------------------------------------------------------------
+struct GraphEntry {
+  const void* q; const float* tau; int32_t k; void* out; float* lse;
+  cudaGraphExec_t exec;
+  uint64_t nodes;
+};
+
+// Complete device-arena layout: the public tables (sekv_layout) plus workspace offsets.
+struct FullLayout {
+  sekv_layout lay;
+  int64_t off_partials1, off_partials2, off_ws_ids, off_ws_count, off_stats, off_chunks, off_bg_chunk,
+      off_zoom_mask, off_items, off_item_span, off_layer_step, off_seg_flag, off_seg_flag2, off_seg_len,
+      off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag;
+  int mask_words, max_chunks;
+  size_t total;
+};
+
+struct sekv_handle {
+  sekv_config cfg;
+  int G, esize;
+  uint8_t* dev; size_t dev_bytes;
+  uint8_t* host; size_t host_bytes;
+  uint8_t* host_dev;                 // device alias of the pinned host arena
+  bool registered_host;
+  sekv_layout lay;
+  FullLayout F;
+  int mask_words;
+  cudaStream_t main, side;
+  bool own_side;
+  cudaEvent_t ev_fork, ev_join;
+  // batch state
+  int n_seqs; bool segmented;
+  std::vector<int> m_b, A_b;
+  std::vector<int64_t> tok_off;
+  std::vector<int32_t> span_len_host;
+  int m_tot, A_tot, max_m;
+  std::vector<char> layer_built;
+  size_t host_used;
+  // schedule
+  int n_chunks, parts1_max, P2, parts_per_head, sort_n;
+  int num_sms;
+  std::vector<GraphEntry> graphs;
+  uint64_t launches;
+  std::string err;
+};
+
+namespace sekv {
+
+inline Dims make_dims(const sekv_handle* h) {
+  Dims d;
+  d.L = h->cfg.n_layers; d.Hq = h->cfg.n_q_heads; d.Hkv = h->cfg.n_kv_heads; d.G = h->G;
+  d.dp = h->cfg.route_dim; d.B = h->n_seqs; d.k_cap = h->cfg.k_cap; d.ways = h->cfg.cache_ways;
+  d.mask_words = h->mask_words;
+  d.rows_cap = (int)h->lay.rows_cap; d.spans_cap = (int)h->lay.spans_cap; d.esize = h->esize;
+  d.slot_bytes = h->lay.slot_bytes;
+  d.parts1_max = h->parts1_max; d.P2 = h->P2; d.parts_per_head = h->parts_per_head;
+  return d;
+}
+
+CsrView csr_view(const sekv_handle* h);
+LayerView layer_view(const sekv_handle* h, int layer);
+
+// launchers (each returns the cudaError_t of the launch)
+cudaError_t launch_segment(sekv_handle* h, const float* H, int n_seqs, const int64_t* tok_off_host,
+                           int* m_out, int* a_out, std::string* why);
+cudaError_t launch_build_prefactored(sekv_handle* h, int layer, const float* H, const sekv_factors* f,
+                                     const void* W);
+cudaError_t launch_build_dense(sekv_handle* h, int layer, const float* H, const void* K, const void* V,
+                               const void* W, int rank_cap, std::string* why);
+cudaError_t launch_route(sekv_handle* h, int layer, const void* q, const float* tau, int k, float* logits,
+                         float* alpha, int32_t* ids, int32_t* count, cudaStream_t s);
+cudaError_t launch_plan(sekv_handle* h, int layer, const int32_t* ids, const int32_t* count, cudaStream_t s);
+cudaError_t launch_fetch(sekv_handle* h, int layer, const int32_t* count, cudaStream_t s);
+cudaError_t launch_stage1(sekv_handle* h, int layer, const void* q, cudaStream_t s);
+cudaError_t launch_stage2(sekv_handle* h, int layer, const void* q, const int32_t* count, cudaStream_t s);
+cudaError_t launch_combine(sekv_handle* h, int layer, void* out, float* lse, cudaStream_t s);
+
+inline uint8_t* ws(const sekv_handle* h, int64_t off) { return h->dev + off; }
+
+}  // namespace sekv

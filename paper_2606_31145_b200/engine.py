@@ -1,0 +1,88 @@
+"""Harness-side setup helper: size a sekv_config for a workload, create the handle, and stage the
+generator's tensors through sekv_build_spans / sekv_build_spans_prefactored layer by layer.
+No arithmetic of the method lives here -- only sizing, allocation and calls through the C ABI."""
+from __future__ import annotations
+
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+
+def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Optional[int] = None,
+               out_dtype: str = "f32", use_graph: int = 0, impl: int = 0, stage1_ctas: int = 0,
+               r_max: Optional[int] = None, slack: float = 1.0) -> B.sekv_config:
+    m_tot = sum(l.m for l in layouts)
+    a_tot = sum(l.A for l in layouts)
+    n_tot = sum(l.n for l in layouts)
+    max_m = max(l.m for l in layouts)
+    max_len = max(int(l.planted_span_len.max()) if l.m else 1 for l in layouts)
+    if k_cap is None:
+        k_cap = max_m if spec.top_k < 0 else spec.top_k
+    if cache_ways is None:
+        cache_ways = max(2 * k_cap, 1) if spec.top_k >= 0 else max(k_cap, 1)
+    return B.make_config(
+        n_layers=spec.n_layers, n_q_heads=spec.n_q_heads, n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim,
+        route_dim=spec.route_dim, dtype=B.SEKV_BF16 if spec.dtype == "bf16" else B.SEKV_F32,
+        out_dtype=B.SEKV_BF16 if out_dtype == "bf16" else B.SEKV_F32, alpha=spec.alpha, l_min=spec.l_min,
+        r_max=r_max or spec.rank, window=spec.window, max_seqs=len(layouts), max_tokens_total=n_tot,
+        max_spans_total=int(m_tot * slack) + 1, max_full_total=int(a_tot * slack) + 1,
+        max_span_len=min(1024, -(-max(max_len, 16) // 16) * 16), k_cap=k_cap, cache_ways=max(cache_ways, 1),
+        stage1_ctas=stage1_ctas, use_graph=use_graph, impl=impl)
+
+
+def host_bytes_for(spec, layouts, cfg: B.sekv_config) -> int:
+    total = 0
+    for l in layouts:
+        for ln in l.planted_span_len:
+            r = min(spec.rank, int(ln))
+            total += B.sekv_blob_bytes(cfg.dtype, int(ln), r, r)
+    return total * spec.n_kv_heads * spec.n_layers + (1 << 16)
+
+
+def seq_tok_off(layouts) -> list:
+    off = [0]
+    for l in layouts:
+        off.append(off[-1] + l.n)
+    return off
+
+
+def build_layer_prefactored(eng: B.Sekv, spec, layouts, li, H_dev: torch.Tensor):
+    eng.sekv_build_spans_prefactored(
+        li.layer, seq_tok_off(layouts), H_dev, rank_in=spec.rank, tokUK=li.tokUK, SK=li.SK, VtK=li.VtK,
+        tokUV=li.tokUV, SV=li.SV, VtV=li.VtV, Kfull=li.Kfull, Vfull=li.Vfull, W=li.W, rank_k=li.rank_k,
+        rank_v=li.rank_v, a_tot=sum(l.A for l in layouts), m_tot=sum(l.m for l in layouts))
+
+
+def surprisal_device(layouts, device) -> torch.Tensor:
+    return torch.from_numpy(np.concatenate([l.H for l in layouts]).astype(np.float32)).to(device)
+
+
+def create_engine(spec, layouts, device="cuda:0", mode: str = "prefactored", gen_device: Optional[str] = None,
+                  layer_inputs: Optional[Sequence] = None, **cfg_kw) -> B.Sekv:
+    """Create a handle sized for `spec` and build every layer from the seeded generator."""
+    from workloads import make_layer_inputs
+    cfg = config_for(spec, layouts, **cfg_kw)
+    eng = B.Sekv(cfg, host_bytes_for(spec, layouts, cfg), device=device)
+    H_dev = surprisal_device(layouts, eng.device)
+    gdev = gen_device or "cpu"
+    for layer in range(spec.n_layers):
+        li = layer_inputs[layer] if layer_inputs is not None else make_layer_inputs(
+            spec, layouts, layer, device=gdev, dense=(mode == "dense"))
+        li = to_device(li, eng.device)
+        if mode == "dense":
+            eng.sekv_build_spans(layer, seq_tok_off(layouts), H_dev, li.K, li.V, li.W, rank_cap=cfg.r_max)
+        else:
+            build_layer_prefactored(eng, spec, layouts, li, H_dev)
+    return eng
+
+
+def to_device(li, device):
+    import dataclasses
+    kw = {}
+    for f in dataclasses.fields(li):
+        v = getattr(li, f.name)
+        kw[f.name] = v.to(device).contiguous() if isinstance(v, torch.Tensor) else v
+    return type(li)(**kw)
