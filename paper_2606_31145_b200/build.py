@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsekv.so")
-STAMP = os.path.join(HERE, "build", "libsekv.stamp")
+STAMP = os.path.join(HERE, "libsekv.stamp")
 SOURCES = ["sekv_api.cu", "build_kernels.cu", "route_kernels.cu", "attn_kernels.cu", "attn_mma_kernels.cu"]
 HEADERS = ["sekv_internal.cuh", "svd_kernels.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

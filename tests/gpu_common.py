@@ -40,7 +40,8 @@ def assert_stored_close(got: np.ndarray, ref: np.ndarray, dtype: str, what: str,
         # near zero, cancellation in the fp32 accumulation is relative to the row's magnitude
         tol = np.maximum(tol, 2e-6 * np.abs(ref).max())
     else:
-        tol = 4e-6 * np.maximum(np.abs(ref), np.abs(ref).max() * 1e-2) + 1e-30
+        # fp32 storage: fp32 accumulation of up to |S| products vs the oracle's fp64
+        tol = 1e-5 * np.abs(ref) + 5e-6 * np.abs(ref).max() + 1e-30
     bad = np.abs(got - ref) > tol
     assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} differ, worst {np.abs(got - ref).max():.3e}"
 
