@@ -9,9 +9,12 @@
 //
 //   QK^T : lane (gid = lane/4, t4 = lane%4) loads 16-byte chunk (t4 + 4j) of the K row of token gid;
 //          its four 32-bit words are the (b0,b1) pairs of two k-steps; Q is loaded the same way.
-//   P V  : lane loads chunk (gid + 8s) of rows 2*t4, 2*t4+1, 2*t4+8, 2*t4+9 of V and builds the
-//          token-pair B fragments with one PRMT per word; output column gid of n-tile (s,e) is
-//          dimension 64s + 8gid + e.
+//   P V  : computed transposed, O^T = V^T P^T (M = 16 dims, N = 8 heads, K = 16 tokens): the C fragment
+//          of S (row = head gid, cols = tokens 2*t4, 2*t4+1) IS the B fragment of P^T (n = gid,
+//          k = 2*t4, 2*t4+1), so no data movement is needed between the two products.  Lane loads
+//          chunk (gid + 8s) of rows 2*t4, 2*t4+1, 2*t4+8, 2*t4+9 of V and builds the token-pair A
+//          fragments with one PRMT per word; rows gid / gid+8 of m-tile (s,w) are dimensions
+//          64s + 8gid + 2w and + 1.
 //   P (fp32) is split into bf16 hi + lo parts and multiplied twice, so probabilities carry ~16 bits.
 //
 // Stage 2 applies the query through the factored form with the same machinery:
@@ -30,6 +33,14 @@ __device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a2
   asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
       : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
       : "r"(a0), "r"(z), "r"(a2), "r"(z), "r"(b0), "r"(b1));
+}
+
+// general form (all four A registers): used for O^T = V^T P^T where the 16 rows are dimensions
+__device__ __forceinline__ void mma16816_full(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                              uint32_t b0, uint32_t b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
 __device__ __forceinline__ uint4 ldg16(const void* p) {
@@ -125,11 +136,12 @@ stage1_mma_kernel(CsrView cv, LayerView lv, const Chunk* __restrict__ chunks, co
     qf[j][0] = v.x; qf[j][1] = v.y; qf[j][2] = v.z; qf[j][3] = v.w;
   }
   float m_run = -INFINITY, l_run = 0.f;
-  float acc[2][8][4];
+  // acc[s][w][2o + c] = O[head 2*t4 + c][dim 64s + 8gid + 2w + o]
+  float acc[2][4][4];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
 #pragma unroll
-    for (int e = 0; e < 8; ++e) { acc[s][e][0] = 0.f; acc[s][e][1] = 0.f; acc[s][e][2] = 0.f; acc[s][e][3] = 0.f; }
+    for (int w = 0; w < 4; ++w) { acc[s][w][0] = 0.f; acc[s][w][1] = 0.f; acc[s][w][2] = 0.f; acc[s][w][3] = 0.f; }
 
   const int ntiles = (row_end - ck.row_begin + 15) >> 4;
   uint4 kf[2][4], vf[4][2];
@@ -194,21 +206,23 @@ stage1_mma_kernel(CsrView cv, LayerView lv, const Chunk* __restrict__ chunks, co
     const float m_new = fmaxf(m_run, mx);
     const float m_safe = (m_new == -INFINITY) ? 0.f : m_new;
     if (__any_sync(0xffffffffu, m_new > m_run)) {
-      const float corr = exp2f(m_run - m_safe);
+      const float corr = exp2f(m_run - m_safe);         // this lane's head is gid
       l_run *= corr;
+      const float ca = __shfl_sync(0xffffffffu, corr, 8 * t4);       // head 2*t4   (lane gid = 2*t4, t4 = 0)
+      const float cb = __shfl_sync(0xffffffffu, corr, 8 * t4 + 4);   // head 2*t4+1
 #pragma unroll
       for (int s = 0; s < 2; ++s)
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { acc[s][e][0] *= corr; acc[s][e][1] *= corr; }
+        for (int w = 0; w < 4; ++w) { acc[s][w][0] *= ca; acc[s][w][1] *= cb; acc[s][w][2] *= ca; acc[s][w][3] *= cb; }
     }
     m_run = m_new;
     const float p00 = exp2f(z[0][0] - m_safe), p01 = exp2f(z[0][1] - m_safe);
     const float p10 = exp2f(z[1][0] - m_safe), p11 = exp2f(z[1][1] - m_safe);
     l_run += (p00 + p01) + (p10 + p11);
-    uint32_t a0h, a0l, a2h, a2l;
-    split_bf16(p00, p01, a0h, a0l);
-    split_bf16(p10, p11, a2h, a2l);
-    // O += P V over 16 n-tiles of 8 dims
+    uint32_t b0h, b0l, b1h, b1l;          // P^T fragments: n = head gid, k = tokens 2*t4+e (b0) and 8+2*t4+e (b1)
+    split_bf16(p00, p01, b0h, b0l);
+    split_bf16(p10, p11, b1h, b1l);
+    // O^T += V^T P^T over 8 m-tiles of 16 dims
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
       const uint32_t ra[4] = {vf[0][s].x, vf[0][s].y, vf[0][s].z, vf[0][s].w};
@@ -217,28 +231,30 @@ stage1_mma_kernel(CsrView cv, LayerView lv, const Chunk* __restrict__ chunks, co
       const uint32_t rd[4] = {vf[3][s].x, vf[3][s].y, vf[3][s].z, vf[3][s].w};
 #pragma unroll
       for (int w = 0; w < 4; ++w) {
-        const uint32_t b0e = __byte_perm(ra[w], rb[w], 0x5410), b1e = __byte_perm(rc[w], rd[w], 0x5410);
-        const uint32_t b0o = __byte_perm(ra[w], rb[w], 0x7632), b1o = __byte_perm(rc[w], rd[w], 0x7632);
-        mma16816(acc[s][2 * w], a0h, a2h, b0e, b1e);
-        mma16816(acc[s][2 * w], a0l, a2l, b0e, b1e);
-        mma16816(acc[s][2 * w + 1], a0h, a2h, b0o, b1o);
-        mma16816(acc[s][2 * w + 1], a0l, a2l, b0o, b1o);
+        const uint32_t a0 = __byte_perm(ra[w], rb[w], 0x5410), a1 = __byte_perm(ra[w], rb[w], 0x7632);
+        const uint32_t a2 = __byte_perm(rc[w], rd[w], 0x5410), a3 = __byte_perm(rc[w], rd[w], 0x7632);
+        mma16816_full(acc[s][w], a0, a1, a2, a3, b0h, b1h);
+        mma16816_full(acc[s][w], a0, a1, a2, a3, b0l, b1l);
       }
     }
     if (more) load_v(t + NW);
   }
-  // warp result -> shared memory.  acc[s][e][c] is head gid, dimension 64s + 16*t4 + 8c + e.
+  // warp result -> shared memory
   l_run = quad_sum(l_run);
-  if (gid < G) {
-    if (t4 == 0) { sm_ml[(warp * G + gid) * 2] = m_run; sm_ml[(warp * G + gid) * 2 + 1] = l_run; }
-    float* o = sm_o + (warp * G + gid) * kD;
+  if (gid < G && t4 == 0) { sm_ml[(warp * G + gid) * 2] = m_run; sm_ml[(warp * G + gid) * 2 + 1] = l_run; }
 #pragma unroll
-    for (int s = 0; s < 2; ++s)
+  for (int c = 0; c < 2; ++c) {
+    const int hh = 2 * t4 + c;
+    if (hh < G) {
+      float* o = sm_o + (warp * G + hh) * kD;
 #pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        o[64 * s + 16 * t4 + e] = acc[s][e][0];
-        o[64 * s + 16 * t4 + 8 + e] = acc[s][e][1];
-      }
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+          o[64 * s + 8 * gid + 2 * w] = acc[s][w][c];
+          o[64 * s + 8 * gid + 2 * w + 1] = acc[s][w][2 + c];
+        }
+    }
   }
   cta_merge_store<G, NW>(sm_o, sm_ml, partials + (size_t)blockIdx.x * G * kPartStride);
 }
