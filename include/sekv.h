@@ -248,6 +248,14 @@ SEKV_API sekv_status sekv_cache_flush(sekv_handle* h);                          
  * summaries + 4m, pool rows, q and out, W; coarse rows are counted in full (the per-step
  * correction for skipped coarse rows and the factor bytes come from sekv_stats). HOST out. */
 SEKV_API sekv_status sekv_static_bytes_per_layer(const sekv_handle* h, uint64_t* bytes);
+/* Per-kernel timing with CUDA events recorded on the launching stream around every kernel of
+ * sekv_route / sekv_decode_attn / sekv_decode_step (non-graph launches only; a graph replay is not
+ * instrumented).  Classes: 0 route (a1-a3), 1 plan (a4 residency), 2 fetch (a4 copy, side stream),
+ * 3 stage 1 (a5), 4 stage 2 (a6), 5 combine (a7).  sekv_get_kernel_times synchronises, writes the
+ * summed milliseconds and launch counts per class since the last call (HOST arrays of 6) and clears. */
+#define SEKV_N_KERNEL_CLASSES 6
+SEKV_API sekv_status sekv_set_profiling(sekv_handle* h, int32_t on);
+SEKV_API sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t* launches);
 /* Number of stage-1 work chunks (CTAs) and partial slots per query head; HOST outs. */
 SEKV_API sekv_status sekv_get_schedule(const sekv_handle* h, int32_t* stage1_ctas, int32_t* parts_per_head);
 

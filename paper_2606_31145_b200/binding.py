@@ -93,10 +93,13 @@ def _load() -> C.CDLL:
     lib.sekv_cache_flush.argtypes = [VP]
     lib.sekv_static_bytes_per_layer.argtypes = [VP, P(C.c_uint64)]
     lib.sekv_get_schedule.argtypes = [VP, P(I32), P(I32)]
+    lib.sekv_set_profiling.argtypes = [VP, I32]
+    lib.sekv_get_kernel_times.argtypes = [VP, P(C.c_double), P(C.c_uint64)]
     for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
-                 "sekv_static_bytes_per_layer", "sekv_get_schedule"):
+                 "sekv_static_bytes_per_layer", "sekv_get_schedule", "sekv_set_profiling",
+                 "sekv_get_kernel_times"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -144,6 +147,20 @@ def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
     return t.data_ptr()
 
 
+_MAIN_STREAMS: dict = {}
+
+
+def main_stream(device: torch.device) -> "torch.cuda.Stream":
+    """One non-default stream per device, made torch's current stream: the library launches on it (and
+    can capture CUDA graphs on it, which the legacy default stream does not allow), and torch ops
+    issued by the caller are ordered with the library's kernels because they share the stream."""
+    key = torch.device(device).index or 0
+    if key not in _MAIN_STREAMS:
+        _MAIN_STREAMS[key] = torch.cuda.Stream(device)
+    torch.cuda.set_stream(_MAIN_STREAMS[key])
+    return _MAIN_STREAMS[key]
+
+
 class Sekv:
     """Owner of one sekv_handle plus the two arenas it borrows.  Method names follow the C calls."""
 
@@ -151,7 +168,8 @@ class Sekv:
         self.cfg = cfg
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self._main = torch.cuda.current_stream(self.device)
+        torch.cuda.synchronize(self.device)
+        self._main = main_stream(self.device)
         self._side = torch.cuda.Stream(self.device)
         cfg.main_stream = self._main.cuda_stream
         cfg.side_stream = self._side.cuda_stream
@@ -284,6 +302,16 @@ class Sekv:
         v = C.c_uint64(0)
         self._check(lib.sekv_static_bytes_per_layer(self._h, C.byref(v)), "sekv_static_bytes_per_layer")
         return int(v.value)
+
+    KERNEL_CLASSES = ("route", "plan", "fetch", "stage1", "stage2", "combine")
+
+    def sekv_set_profiling(self, on: bool):
+        self._check(lib.sekv_set_profiling(self._h, 1 if on else 0), "sekv_set_profiling")
+
+    def sekv_get_kernel_times(self) -> dict:
+        ms, n = (C.c_double * 6)(), (C.c_uint64 * 6)()
+        self._check(lib.sekv_get_kernel_times(self._h, ms, n), "sekv_get_kernel_times")
+        return {name: dict(ms=float(ms[i]), launches=int(n[i])) for i, name in enumerate(self.KERNEL_CLASSES)}
 
     def sekv_get_schedule(self):
         a, b = C.c_int32(0), C.c_int32(0)

@@ -247,6 +247,7 @@ sekv_status sekv_create(const sekv_config* cfg, void* device_arena, size_t devic
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
   h->launches = 0;
+  h->profiling = false;
   *out = h;
   sekv_status s = sekv_reset(h);
   if (s != SEKV_OK) { sekv_destroy(h); *out = nullptr; return s; }
@@ -258,6 +259,7 @@ void sekv_destroy(sekv_handle* h) {
   cudaStreamSynchronize(h->main);
   cudaStreamSynchronize(h->side);
   for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+  for (auto& r : h->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   if (h->own_side) cudaStreamDestroy(h->side);
   cudaEventDestroy(h->ev_fork);
   cudaEventDestroy(h->ev_join);
@@ -496,6 +498,24 @@ sekv_status sekv_build_spans(sekv_handle* h, int32_t layer, int32_t n_seqs, cons
 }
 
 // ---- decode --------------------------------------------------------------------------------------------
+// CUDA-event bracket around one kernel launch when profiling is on (never during graph capture)
+struct ProfScope {
+  sekv_handle* h; cudaStream_t s; int idx;
+  ProfScope(sekv_handle* h_, int cls, cudaStream_t s_) : h(h_), s(s_), idx(-1) {
+    if (!h->profiling) return;
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone) return;
+    sekv_handle::ProfRec r;
+    r.cls = cls;
+    if (cudaEventCreate(&r.a) != cudaSuccess) return;
+    if (cudaEventCreate(&r.b) != cudaSuccess) { cudaEventDestroy(r.a); return; }
+    cudaEventRecord(r.a, s);
+    h->prof.push_back(r);
+    idx = (int)h->prof.size() - 1;
+  }
+  ~ProfScope() { if (idx >= 0) cudaEventRecord(h->prof[idx].b, s); }
+};
+
 static sekv_status check_ready(sekv_handle* h, int layer) {
   if (!h->segmented) return fail(h, SEKV_STATE, "no sequences built");
   if (layer < 0 || layer >= h->cfg.n_layers) return fail(h, SEKV_INVALID_ARG, "layer out of range");
@@ -516,7 +536,8 @@ sekv_status sekv_route(sekv_handle* h, int32_t layer, const void* q, const float
   if (s != SEKV_OK) return s;
   if (!q || !ids || !count) return fail(h, SEKV_INVALID_ARG, "q, ids or count is NULL");
   if ((s = check_k(h, k)) != SEKV_OK) return s;
-  cudaError_t e = launch_route(h, layer, q, tau, k, logits, alpha_tilde, ids, count, h->main);
+  cudaError_t e;
+  { ProfScope ps(h, 0, h->main); e = launch_route(h, layer, q, tau, k, logits, alpha_tilde, ids, count, h->main); }
   if (e != cudaSuccess) return cuda_fail(h, e, "route");
   return SEKV_OK;
 }
@@ -524,18 +545,20 @@ sekv_status sekv_route(sekv_handle* h, int32_t layer, const void* q, const float
 static cudaError_t decode_layer(sekv_handle* h, int layer, const void* q, const int32_t* ids, const int32_t* count,
                                 void* out, float* lse) {
   cudaError_t e;
-  if ((e = launch_plan(h, layer, ids, count, h->main)) != cudaSuccess) return e;
+  { ProfScope ps(h, 1, h->main); if ((e = launch_plan(h, layer, ids, count, h->main)) != cudaSuccess) return e; }
   if (h->cfg.k_cap > 0) {
     if ((e = cudaEventRecord(h->ev_fork, h->main)) != cudaSuccess) return e;
     if ((e = cudaStreamWaitEvent(h->side, h->ev_fork, 0)) != cudaSuccess) return e;
-    if ((e = launch_fetch(h, layer, count, h->side)) != cudaSuccess) return e;
+    { ProfScope ps(h, 2, h->side); if ((e = launch_fetch(h, layer, count, h->side)) != cudaSuccess) return e; }
     if ((e = cudaEventRecord(h->ev_join, h->side)) != cudaSuccess) return e;
   }
-  if ((e = launch_stage1(h, layer, q, h->main)) != cudaSuccess) return e;
+  { ProfScope ps(h, 3, h->main); if ((e = launch_stage1(h, layer, q, h->main)) != cudaSuccess) return e; }
   if (h->cfg.k_cap > 0) {
     if ((e = cudaStreamWaitEvent(h->main, h->ev_join, 0)) != cudaSuccess) return e;
+    ProfScope ps(h, 4, h->main);
     if ((e = launch_stage2(h, layer, q, count, h->main)) != cudaSuccess) return e;
   }
+  ProfScope ps(h, 5, h->main);
   return launch_combine(h, layer, out, lse, h->main);
 }
 
@@ -563,6 +586,7 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
     int32_t* cnt = (int32_t*)(h->dev + h->F.off_ws_count) + (size_t)l * c.max_seqs * c.n_kv_heads;
     cudaError_t e;
     if (c.k_cap > 0) {
+      ProfScope ps(h, 0, h->main);
       e = launch_route(h, l, ql, tau ? tau + (size_t)l * c.n_q_heads : nullptr, k, nullptr, nullptr, ids, cnt, h->main);
       if (e != cudaSuccess) return e;
     }
@@ -580,7 +604,7 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   if (!q || !out) return fail(h, SEKV_INVALID_ARG, "q or out is NULL");
   sekv_status s = check_k(h, k);
   if (s != SEKV_OK) return s;
-  if (!h->cfg.use_graph) {
+  if (!h->cfg.use_graph || h->profiling) {   // profiling brackets kernels with events: eager launches only
     cudaError_t e = enqueue_step(h, q, tau, k, out, lse);
     if (e != cudaSuccess) return cuda_fail(h, e, "decode_step");
     return SEKV_OK;
@@ -679,6 +703,31 @@ sekv_status sekv_static_bytes_per_layer(const sekv_handle* h, uint64_t* bytes) {
     t += (uint64_t)c.n_q_heads * kD * (b + bo);                 // q and out
   }
   *bytes = t;
+  return SEKV_OK;
+}
+
+static void prof_clear(sekv_handle* h) {
+  for (auto& r : h->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  h->prof.clear();
+}
+
+sekv_status sekv_set_profiling(sekv_handle* h, int32_t on) {
+  if (!h) return SEKV_INVALID_ARG;
+  h->profiling = on != 0;
+  return SEKV_OK;
+}
+
+sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t* launches) {
+  if (!h || !ms || !launches) return SEKV_INVALID_ARG;
+  CK(h, cudaStreamSynchronize(h->main));
+  CK(h, cudaStreamSynchronize(h->side));
+  for (int i = 0; i < SEKV_N_KERNEL_CLASSES; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  for (auto& r : h->prof) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) { ms[r.cls] += t; launches[r.cls] += 1; }
+  }
+  cudaGetLastError();
+  prof_clear(h);
   return SEKV_OK;
 }
 

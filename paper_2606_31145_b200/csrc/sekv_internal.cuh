@@ -175,6 +175,10 @@ struct sekv_handle {
   int num_sms;
   std::vector<GraphEntry> graphs;
   uint64_t launches;
+  // per-kernel-class CUDA-event timing (sekv_set_profiling)
+  bool profiling;
+  struct ProfRec { int cls; cudaEvent_t a, b; };
+  std::vector<ProfRec> prof;
   std::string err;
 };
 

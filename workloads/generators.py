@@ -134,12 +134,15 @@ def _orthonormal_columns(a: torch.Tensor) -> torch.Tensor:
     if not a.is_cuda:
         q, _ = torch.linalg.qr(a, mode="reduced")
         return q
-    q = a
+    q = a.to(torch.float64)
+    eye = torch.eye(a.shape[-1], device=a.device, dtype=torch.float64)
     for _ in range(2):
         g = q.transpose(-1, -2) @ q
+        # tiny relative shift keeps near-singular Gram matrices factorisable; the 2nd pass removes its effect
+        g = g + eye * (1e-13 * g.diagonal(dim1=-2, dim2=-1).sum(-1)[..., None, None])
         l = torch.linalg.cholesky(g)
         q = torch.linalg.solve_triangular(l, q.transpose(-1, -2), upper=False).transpose(-1, -2)
-    return q
+    return q.to(a.dtype)
 
 
 def _span_factors(gen: torch.Generator, lens: torch.Tensor, rows_pad: int, r: int, device,
