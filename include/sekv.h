@@ -83,10 +83,14 @@ typedef struct sekv_config {
   int32_t max_full_total;    /* capacity of sum_b A_b (anchors + short runs + window) */
   int32_t max_span_len;      /* <= SEKV_MAX_SPAN_LEN; longer runs make build fail UNSUPPORTED */
   int32_t k_cap;             /* max zoomed spans per (sequence, kv head) and step */
-  int32_t cache_ways;        /* device factor-cache slots per (layer, sequence, kv head), >= k_cap */
-  int32_t stage1_ctas;       /* 0 = auto (multiple of the SM count) */
+  int32_t cache_ways;        /* device factor-cache slots per (layer, sequence, kv head), >= k_cap + prefetch */
+  int32_t prefetch;          /* speculative prefetch depth: after each layer-step the `prefetch` next-best spans by
+                                routing score that are not resident are copied host -> cache on the side stream */
+  int32_t stage1_ctas;       /* generic path: stage-1 grid; 0 = auto (multiple of the SM count) */
+  int32_t item_rows;         /* fused path: entry rows per POOL / COARSE work item, multiple of 16; 0 = auto */
+  int32_t zoom_spans_per_item; /* fused path: expanded spans per ZOOM work item; 0 = auto (4) */
   int32_t use_graph;         /* 1: sekv_decode_step replays a captured CUDA graph */
-  int32_t impl;              /* 0 = auto (tensor-core kernels for bf16), 1 = force the generic kernels */
+  int32_t impl;              /* 0 = auto (bf16: the fused layer kernel), 1 = force the generic multi-kernel path */
   void* main_stream;         /* cudaStream_t; NULL = legacy default stream */
   void* side_stream;         /* cudaStream_t for the factor fetch; NULL = created by the library */
 } sekv_config;
@@ -134,6 +138,7 @@ typedef struct sekv_stats {
   uint64_t h2d_bytes;            /* factor bytes fetched host -> device cache */
   uint64_t factor_bytes_algo;    /* sum over expansions of (r_K+r_V)(|S|+d_h) b + 4(r_K+r_V): Eq. 18 with fp32 sigma */
   uint64_t coarse_rows_skipped;  /* coarse entries replaced by their tokens (= zoomed_spans) */
+  uint64_t prefetched_spans;     /* blobs copied by the side-stream prefetch (their bytes are in h2d_bytes) */
   uint64_t kernel_launches;      /* kernels launched or graph nodes replayed by this handle */
 } sekv_stats;
 
@@ -234,6 +239,10 @@ SEKV_API sekv_status sekv_decode_attn(sekv_handle* h, int32_t layer, const void*
 SEKV_API sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out,
                              float* lse);
 
+/* Zoom sets chosen by the last sekv_decode_step for `layer`: copies ids [B][H_kv][k_cap] and count
+ * [B][H_kv] (DEVICE int32 outputs, same format as sekv_route) on the main stream. */
+SEKV_API sekv_status sekv_last_zoom_ids(sekv_handle* h, int32_t layer, int32_t* ids, int32_t* count);
+
 /* Same through HOST buffers (pinned recommended): copies q host->device, runs the step, copies
  * out (and lse if not NULL) device->host, and waits for completion.  tau stays a DEVICE pointer. */
 SEKV_API sekv_status sekv_decode_step_host(sekv_handle* h, const void* q_host, const float* tau, int32_t k,
@@ -251,9 +260,11 @@ SEKV_API sekv_status sekv_static_bytes_per_layer(const sekv_handle* h, uint64_t*
 /* Per-kernel timing with CUDA events recorded on the launching stream around every kernel of
  * sekv_route / sekv_decode_attn / sekv_decode_step (non-graph launches only; a graph replay is not
  * instrumented).  Classes: 0 route (a1-a3), 1 plan (a4 residency), 2 fetch (a4 copy, side stream),
- * 3 stage 1 (a5), 4 stage 2 (a6), 5 combine (a7).  sekv_get_kernel_times synchronises, writes the
- * summed milliseconds and launch counts per class since the last call (HOST arrays of 6) and clears. */
-#define SEKV_N_KERNEL_CLASSES 6
+ * 3 stage 1 (a5), 4 stage 2 (a6), 5 combine (a7) -- the generic multi-kernel path -- and 6 the fused
+ * layer kernel (a1-a7 in one launch, bf16 path), 7 the side-stream prefetch copy.
+ * sekv_get_kernel_times synchronises, writes the summed milliseconds and launch counts per class since
+ * the last call (HOST arrays of SEKV_N_KERNEL_CLASSES) and clears. */
+#define SEKV_N_KERNEL_CLASSES 8
 SEKV_API sekv_status sekv_set_profiling(sekv_handle* h, int32_t on);
 SEKV_API sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t* launches);
 /* Number of stage-1 work chunks (CTAs) and partial slots per query head; HOST outs. */

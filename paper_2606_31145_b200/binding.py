@@ -32,7 +32,8 @@ class sekv_config(C.Structure):
                 ("out_dtype", C.c_int32), ("alpha", C.c_float), ("l_min", C.c_int32), ("r_max", C.c_int32),
                 ("window", C.c_int32), ("max_seqs", C.c_int32), ("max_tokens_total", C.c_int64),
                 ("max_spans_total", C.c_int32), ("max_full_total", C.c_int32), ("max_span_len", C.c_int32),
-                ("k_cap", C.c_int32), ("cache_ways", C.c_int32), ("stage1_ctas", C.c_int32),
+                ("k_cap", C.c_int32), ("cache_ways", C.c_int32), ("prefetch", C.c_int32),
+                ("stage1_ctas", C.c_int32), ("item_rows", C.c_int32), ("zoom_spans_per_item", C.c_int32),
                 ("use_graph", C.c_int32), ("impl", C.c_int32), ("main_stream", C.c_void_p),
                 ("side_stream", C.c_void_p)]
 
@@ -49,7 +50,7 @@ class sekv_layout(C.Structure):
 
 
 _STATS_FIELDS = ["layer_steps", "zoomed_spans", "cache_hits", "cache_misses", "h2d_bytes", "factor_bytes_algo",
-                 "coarse_rows_skipped", "kernel_launches"]
+                 "coarse_rows_skipped", "prefetched_spans", "kernel_launches"]
 
 
 class sekv_stats(C.Structure):
@@ -87,6 +88,7 @@ def _load() -> C.CDLL:
     lib.sekv_decode_attn.argtypes = [VP, I32, VP, VP, VP, VP, VP]
     lib.sekv_decode_step.argtypes = [VP, VP, VP, I32, VP, VP]
     lib.sekv_decode_step_host.argtypes = [VP, VP, VP, I32, VP, VP]
+    lib.sekv_last_zoom_ids.argtypes = [VP, I32, VP, VP]
     lib.sekv_get_layout.argtypes = [VP, P(sekv_layout)]
     lib.sekv_get_stats.argtypes = [VP, P(sekv_stats)]
     lib.sekv_reset_stats.argtypes = [VP]
@@ -97,6 +99,7 @@ def _load() -> C.CDLL:
     lib.sekv_get_kernel_times.argtypes = [VP, P(C.c_double), P(C.c_uint64)]
     for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
+                 "sekv_last_zoom_ids",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
                  "sekv_static_bytes_per_layer", "sekv_get_schedule", "sekv_set_profiling",
                  "sekv_get_kernel_times"):
@@ -131,8 +134,8 @@ def make_config(**kw) -> sekv_config:
     """Config with the paper's defaults: alpha 1.0, l_min 16, d' 32, R_max 32."""
     d = dict(n_layers=1, n_q_heads=32, n_kv_heads=8, head_dim=128, route_dim=32, dtype=SEKV_BF16,
              out_dtype=SEKV_F32, alpha=1.0, l_min=16, r_max=32, window=0, max_seqs=1, max_tokens_total=1,
-             max_spans_total=1, max_full_total=1, max_span_len=256, k_cap=16, cache_ways=32, stage1_ctas=0,
-             use_graph=0, impl=0, main_stream=None, side_stream=None)
+             max_spans_total=1, max_full_total=1, max_span_len=256, k_cap=16, cache_ways=32, prefetch=0, stage1_ctas=0,
+             item_rows=0, zoom_spans_per_item=0, use_graph=0, impl=0, main_stream=None, side_stream=None)
     unknown = set(kw) - set(d)
     if unknown:
         raise TypeError(f"unknown config fields {sorted(unknown)}")
@@ -274,6 +277,13 @@ class Sekv:
         self._check(st, "sekv_decode_step")
         return out
 
+    def sekv_last_zoom_ids(self, layer: int):
+        kc = max(self.cfg.k_cap, 1)
+        ids = torch.empty((self.n_seqs, self.cfg.n_kv_heads, kc), dtype=torch.int32, device=self.device)
+        count = torch.empty((self.n_seqs, self.cfg.n_kv_heads), dtype=torch.int32, device=self.device)
+        self._check(lib.sekv_last_zoom_ids(self._h, layer, _ptr(ids), _ptr(count)), "sekv_last_zoom_ids")
+        return ids, count
+
     def sekv_decode_step_host(self, q_host: torch.Tensor, k: int, out_host: torch.Tensor,
                               tau: Optional[torch.Tensor] = None, lse_host: Optional[torch.Tensor] = None):
         assert not q_host.is_cuda and not out_host.is_cuda
@@ -303,13 +313,13 @@ class Sekv:
         self._check(lib.sekv_static_bytes_per_layer(self._h, C.byref(v)), "sekv_static_bytes_per_layer")
         return int(v.value)
 
-    KERNEL_CLASSES = ("route", "plan", "fetch", "stage1", "stage2", "combine")
+    KERNEL_CLASSES = ("route", "plan", "fetch", "stage1", "stage2", "combine", "fused", "prefetch")
 
     def sekv_set_profiling(self, on: bool):
         self._check(lib.sekv_set_profiling(self._h, 1 if on else 0), "sekv_set_profiling")
 
     def sekv_get_kernel_times(self) -> dict:
-        ms, n = (C.c_double * 6)(), (C.c_uint64 * 6)()
+        ms, n = (C.c_double * 8)(), (C.c_uint64 * 8)()
         self._check(lib.sekv_get_kernel_times(self._h, ms, n), "sekv_get_kernel_times")
         return {name: dict(ms=float(ms[i]), launches=int(n[i])) for i, name in enumerate(self.KERNEL_CLASSES)}
 

@@ -12,8 +12,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsekv.so")
 STAMP = os.path.join(HERE, "libsekv.stamp")
-SOURCES = ["sekv_api.cu", "build_kernels.cu", "route_kernels.cu", "attn_kernels.cu", "attn_mma_kernels.cu"]
-HEADERS = ["sekv_internal.cuh", "svd_kernels.cuh"]
+SOURCES = ["sekv_api.cu", "build_kernels.cu", "route_kernels.cu", "attn_kernels.cu", "fused_kernels.cu"]
+HEADERS = ["sekv_internal.cuh", "svd_kernels.cuh", "mma_common.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--use_fast_math=false",
               "-I", os.path.join(ROOT, "include"), "-I", CSRC]

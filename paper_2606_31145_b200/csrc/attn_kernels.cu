@@ -1,6 +1,7 @@
-// a5-a7, generic kernels (any storage dtype, plain fp32 ALU math).  These are the reference-grade
-// CUDA path: used for fp32 storage (config 0) and when cfg.impl = 1; the bf16 tensor-core path lives in
-// attn_mma_kernels.cu and is checked against the same oracle.
+// a5-a7, generic kernels (any storage dtype, plain fp32 ALU math), one kernel per step.  Used for fp32
+// storage (config 0), when cfg.impl = 1, and when a factor blob is too large for the fused kernel's
+// shared-memory staging; the bf16 hot path is the fused layer kernel in fused_kernels.cu, checked against
+// the same oracle.
 //
 // Softmax bookkeeping is in the base-2 domain: z = logit * log2(e); a partial is
 // (m2 = max z, l = sum 2^(z - m2), o[128] = sum 2^(z - m2) v), merged by the combine kernel
@@ -11,9 +12,6 @@
 
 namespace sekv {
 
-bool have_mma_kernels();
-cudaError_t launch_stage1_mma(sekv_handle* h, int layer, const void* q, cudaStream_t s);
-cudaError_t launch_stage2_mma(sekv_handle* h, int layer, const void* q, const int32_t* count, cudaStream_t s);
 
 // ---------------------------------------------------------------------------------------------
 // a5: stage 1 -- pool tokens (logit = q.K/sqrt(d)) and unexpanded coarse entries
@@ -120,10 +118,7 @@ static cudaError_t launch_stage1_t(sekv_handle* h, int layer, const void* q, cud
   return cudaGetLastError();
 }
 
-static bool use_mma(const sekv_handle* h) { return have_mma_kernels() && h->cfg.dtype == SEKV_BF16 && h->cfg.impl != 1; }
-
 cudaError_t launch_stage1(sekv_handle* h, int layer, const void* q, cudaStream_t s) {
-  if (use_mma(h)) return launch_stage1_mma(h, layer, q, s);
   if (h->cfg.dtype == SEKV_BF16) return launch_stage1_t<__nv_bfloat16>(h, layer, q, s);
   return launch_stage1_t<float>(h, layer, q, s);
 }
@@ -174,8 +169,7 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
     const float* sV = (const float*)(blob + bd.off_sv);
     const ST* VtK = (const ST*)(blob + bd.off_vtk);
     const ST* VV = (const ST*)(blob + bd.off_vv);
-    const ST* UK = (const ST*)(blob + bd.off_uk);
-    const ST* UVt = (const ST*)(blob + bd.off_uvt);
+    const int es = (int)sizeof(ST);
     // c[h][i]
     for (int o = tid; o < G * bd.rkp; o += kS2Threads) {
       const int h = o / bd.rkp, i = o % bd.rkp;
@@ -199,7 +193,7 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
       for (int h = 0; h < G; ++h) z[h] = 0.f;
       for (int i = 0; i < bd.rkp; i += 4) {
         float u4[4];
-        ld4(UK + (size_t)t * bd.rkp + i, u4);
+        ld4((const ST*)(blob + blob_uk_off(bd, es, t, i)), u4);
 #pragma unroll
         for (int h = 0; h < G; ++h) {
           z[h] = fmaf(u4[0], sh_c[h][i], z[h]); z[h] = fmaf(u4[1], sh_c[h][i + 1], z[h]);
@@ -245,7 +239,7 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
       float a = 0.f;
       for (int t = 0; t < bd.lenp; t += 4) {
         float u4[4];
-        ld4(UVt + (size_t)i * bd.lenp + t, u4);
+        ld4((const ST*)(blob + blob_uv_off(bd, es, t, i)), u4);
         a = fmaf(u4[0], sh_z[h][t], a); a = fmaf(u4[1], sh_z[h][t + 1], a);
         a = fmaf(u4[2], sh_z[h][t + 2], a); a = fmaf(u4[3], sh_z[h][t + 3], a);
       }
@@ -304,7 +298,6 @@ static cudaError_t launch_stage2_t(sekv_handle* h, int layer, const void* q, con
 
 cudaError_t launch_stage2(sekv_handle* h, int layer, const void* q, const int32_t* count, cudaStream_t s) {
   if (h->cfg.k_cap <= 0) return cudaSuccess;
-  if (use_mma(h)) return launch_stage2_mma(h, layer, q, count, s);
   if (h->cfg.dtype == SEKV_BF16) return launch_stage2_t<__nv_bfloat16>(h, layer, q, count, s);
   return launch_stage2_t<float>(h, layer, q, count, s);
 }

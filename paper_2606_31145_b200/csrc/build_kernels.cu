@@ -354,14 +354,27 @@ __global__ void pack_blob_kernel(CsrView cv, sekv_factors f, size_t tok_tot, int
   const ST* vtv = (const ST*)f.VtV + ((size_t)g * m_tot + s) * r * kD;
   ST* bvv = (ST*)(blob + bd.off_vv);
   for (int o = tid; o < kD * bd.rvp; o += nt) { int d = o / bd.rvp, i = o % bd.rvp; bvv[o] = i < rv ? vtv[(size_t)i * kD + d] : zero; }
-  // UK [lenp][rkp]
+  // chunks of 16 tokens: [UK 16 x rkp][UVt rvp x 16]  (UVt = transpose of UV [len][r])
   const ST* uk = (const ST*)f.tokUK + ((size_t)g * tok_tot + tok0) * r;
-  ST* buk = (ST*)(blob + bd.off_uk);
-  for (int o = tid; o < bd.lenp * bd.rkp; o += nt) { int t = o / bd.rkp, i = o % bd.rkp; buk[o] = (t < len && i < rk) ? uk[(size_t)t * r + i] : zero; }
-  // UVt [rvp][lenp] = transpose of UV [len][r]
   const ST* uv = (const ST*)f.tokUV + ((size_t)g * tok_tot + tok0) * r;
-  ST* buvt = (ST*)(blob + bd.off_uvt);
-  for (int o = tid; o < bd.rvp * bd.lenp; o += nt) { int i = o / bd.lenp, t = o % bd.lenp; buvt[o] = (t < len && i < rv) ? uv[(size_t)t * r + i] : zero; }
+  const int per_chunk = kLenPad * (bd.rkp + bd.rvp);
+  ST* bch = (ST*)(blob + bd.off_chunks);
+  for (int o = tid; o < (bd.lenp / kLenPad) * per_chunk; o += nt) {
+    const int c = o / per_chunk, w = o % per_chunk;
+    ST v = zero;
+    if (w < kLenPad * bd.rkp) {
+      const int t = c * kLenPad + w / bd.rkp, i = w % bd.rkp;
+      if (t < len && i < rk) v = uk[(size_t)t * r + i];
+    } else {
+      const int w2 = w - kLenPad * bd.rkp;
+      const int i = w2 / kLenPad, t = c * kLenPad + w2 % kLenPad;
+      if (t < len && i < rv) v = uv[(size_t)t * r + i];
+    }
+    bch[o] = v;
+  }
+  // tail padding up to the 128-byte blob size
+  const size_t used = bd.off_chunks + (size_t)(bd.lenp / kLenPad) * bd.chunk_bytes;
+  for (size_t o = used + tid; o < bd.bytes; o += nt) blob[o] = 0;
 }
 
 template <typename ST>

@@ -42,7 +42,10 @@ const char* check_config(const sekv_config* c) {
   if (c->max_spans_total < 1 || c->max_full_total < 0) return "bad span / pool capacity";
   if (c->max_span_len < 1 || c->max_span_len > SEKV_MAX_SPAN_LEN) return "max_span_len must be in [1, 1024]";
   if (c->k_cap < 0) return "k_cap < 0";
-  if (c->cache_ways < std::max(c->k_cap, 1)) return "cache_ways must be >= max(k_cap, 1)";
+  if (c->prefetch < 0 || c->prefetch > 1024) return "prefetch must be in [0, 1024]";
+  if (c->cache_ways < std::max(c->k_cap, 1) + c->prefetch) return "cache_ways must be >= max(k_cap, 1) + prefetch";
+  if (c->item_rows < 0 || c->item_rows % 16) return "item_rows must be a non-negative multiple of 16";
+  if (c->zoom_spans_per_item < 0 || c->zoom_spans_per_item > 64) return "zoom_spans_per_item must be in [0, 64]";
   if (c->cache_ways > 8192) return "cache_ways > 8192";
   if (c->stage1_ctas < 0 || c->stage1_ctas > 4096) return "stage1_ctas out of range";
   if (!(c->alpha == c->alpha)) return "alpha is NaN";
@@ -56,6 +59,7 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   const int64_t B = c.max_seqs, Hq = c.n_q_heads, Hkv = c.n_kv_heads, NL = c.n_layers;
   const int64_t mcap = c.max_spans_total, acap = c.max_full_total, rcap = mcap + acap;
   const int kcap = std::max(c.k_cap, 1);
+  const int kc = kcap + std::max(c.prefetch, 0);
   L.esize = es; L.rows_cap = rcap; L.spans_cap = mcap;
   Carver cv;
   L.seq_tok_off = cv.take((B + 1) * 8);
@@ -85,7 +89,11 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   L.slot_bytes = (int64_t)bd.bytes;
   L.cache_slots = cv.take((size_t)regions * c.cache_ways * bd.bytes);
   // workspace
-  F->max_chunks = std::max(c.stage1_ctas, 1024) + (int)(B * Hkv);
+  // capacity of the stage-1 chunk list (generic path) and of the fused kernel's item list
+  const int64_t zs_min = std::max<int64_t>(1, c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 4);
+  const int64_t attn_items = Hkv * (rcap / 64 + 2 * B + 2) + B * Hkv * ((kcap + zs_min - 1) / zs_min);
+  F->max_chunks = (int)std::max<int64_t>(std::max(c.stage1_ctas, 1024) + B * Hkv, attn_items);
+  F->max_items = (int)(attn_items + Hkv * (mcap / 256 + B + 1));
   const int G = c.n_q_heads / c.n_kv_heads;
   const int P2 = (kcap + kStage2SpansPerCta - 1) / kStage2SpansPerCta;
   F->off_partials1 = cv.take((size_t)F->max_chunks * G * kPartStride * 4);
@@ -97,8 +105,18 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   F->off_bg_chunk = cv.take((size_t)(B * Hkv + 1) * 4);
   F->mask_words = (int)((std::min<int64_t>(mcap, SEKV_MAX_SPANS_PER_SEQ) + 31) / 32);
   F->off_zoom_mask = cv.take((size_t)NL * B * Hkv * F->mask_words * 4);
-  F->off_items = cv.take((size_t)NL * B * Hkv * kcap * 4);
-  F->off_item_span = cv.take((size_t)NL * B * Hkv * kcap * 4);
+  F->off_items = cv.take((size_t)NL * B * Hkv * kc * 4);
+  F->off_item_span = cv.take((size_t)NL * B * Hkv * kc * 4);
+  F->off_items_sched = cv.take((size_t)F->max_items * sizeof(Item));
+  F->off_bg_part = cv.take((size_t)(B * Hkv + 1) * 4);
+  F->off_bg_route = cv.take((size_t)(B * Hkv) * 4);
+  int kpb = 32;
+  while (kpb < std::min<int64_t>(mcap, SEKV_MAX_SPANS_PER_SEQ)) kpb <<= 1;
+  F->keys_per_bg = kpb;
+  F->off_keys = cv.take((size_t)B * Hkv * kpb * 8);
+  F->ctrs_per_layer = (int)(2 + 3 * B * Hkv);
+  F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);
+  F->off_plan_counts = cv.take((size_t)NL * B * Hkv * 2 * 4);
   F->off_layer_step = cv.take((size_t)NL * 4);
   F->off_seg_flag = cv.take((size_t)c.max_tokens_total);
   F->off_seg_flag2 = cv.take((size_t)c.max_tokens_total);
@@ -152,7 +170,7 @@ LayerView layer_view(const sekv_handle* h, int l) {
   const sekv_layout& L = h->lay;
   const sekv_config& c = h->cfg;
   const int64_t B = c.max_seqs, Hkv = c.n_kv_heads;
-  const int kcap = std::max(c.k_cap, 1);
+  const int kcap = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
   v.ent_k = d + L.ent_k + (int64_t)l * L.ent_layer_stride;
   v.ent_v = d + L.ent_v + (int64_t)l * L.ent_layer_stride;
   v.route = d + L.route + (int64_t)l * L.route_layer_stride;
@@ -284,7 +302,10 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_stats, 0, ST_COUNT * 8, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_err_flag, 0, 16, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
+  h->n_items = h->n_route_items = 0; h->use_fused = false;
   h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
   h->span_len_host.clear();
   h->m_tot = h->A_tot = h->max_m = 0;
@@ -363,6 +384,80 @@ static sekv_status make_schedule(sekv_handle* h) {
   return SEKV_OK;
 }
 
+// Work-item list of the fused layer kernel (bf16 path), in queue order: ROUTE chunks, POOL row ranges,
+// ZOOM item ranges, COARSE row ranges.  A topological order: ZOOM / COARSE items depend on the plan that the
+// last ROUTE chunk of their (sequence, kv head) publishes.
+static sekv_status make_fused_schedule(sekv_handle* h) {
+  const FullLayout& F = h->F;
+  const sekv_config& c = h->cfg;
+  h->use_fused = false;
+  if (c.dtype != SEKV_BF16 || c.impl == 1) return SEKV_OK;
+  const int B = h->n_seqs, Hkv = c.n_kv_heads, BG = B * Hkv;
+  if (h->max_m > SEKV_MAX_SPANS_PER_SEQ) return SEKV_OK;
+  const size_t smem = fused_smem_bytes(h, nullptr);
+  if (smem + 20 * 1024 > 227 * 1024) return SEKV_OK;        // blobs too large to double-buffer: generic path
+  int occ = fused_occupancy(h);
+  cudaGetLastError();
+  if (occ < 1) return SEKV_OK;
+  h->fused_occ = occ;
+  h->fused_grid = occ * h->num_sms;
+  long total_rows = 0;
+  int max_rows = 0;
+  for (int b = 0; b < B; ++b) { total_rows += (long)(h->A_b[b] + h->m_b[b]) * Hkv; max_rows = std::max(max_rows, h->A_b[b] + h->m_b[b]); }
+  int rows = c.item_rows;
+  if (rows <= 0) {
+    rows = (int)((total_rows * 2 + 5L * h->fused_grid - 1) / (5L * h->fused_grid));     // ~2.5 items per resident CTA
+    rows = std::min(256, std::max(64, round_up(rows, 64)));
+  }
+  rows = std::max(rows, round_up((max_rows + 299) / 300, 16));                           // <= ~300 row items per group
+  h->fused_item_rows = rows;
+  const int kcap = std::max(c.k_cap, 1);
+  int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 4;
+  zs = std::max(zs, (kcap + 127) / 128);                                                  // <= 128 zoom items per group
+  std::vector<Item> items;
+  std::vector<int32_t> part_base(BG + 1, 0), route_items(BG, 0), nparts(BG, 0);
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) {
+      const int bg = b * Hkv + g, m = h->m_b[b];
+      int n = 0;
+      for (int s0 = 0; s0 == 0 || s0 < m; s0 += 256, ++n) items.push_back(Item{IT_ROUTE, bg, s0, std::min(m, s0 + 256), 0});
+      route_items[bg] = n;
+    }
+  h->n_route_items = (int)items.size();
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) {
+      const int bg = b * Hkv + g, A = h->A_b[b];
+      for (int r0 = 0; r0 < A; r0 += rows) items.push_back(Item{IT_POOL, bg, r0, std::min(A, r0 + rows), nparts[bg]++});
+    }
+  if (c.k_cap > 0)
+    for (int b = 0; b < B; ++b)
+      for (int g = 0; g < Hkv; ++g) {
+        const int bg = b * Hkv + g;
+        const int kmax = std::min(c.k_cap, h->m_b[b]);
+        for (int j0 = 0; j0 < kmax; j0 += zs) items.push_back(Item{IT_ZOOM, bg, j0, std::min(kmax, j0 + zs), nparts[bg]++});
+      }
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) {
+      const int bg = b * Hkv + g, A = h->A_b[b], R = h->A_b[b] + h->m_b[b];
+      for (int r0 = A; r0 < R; r0 += rows) items.push_back(Item{IT_COARSE, bg, r0, std::min(R, r0 + rows), nparts[bg]++});
+    }
+  int total_parts = 0;
+  for (int bg = 0; bg < BG; ++bg) {
+    part_base[bg] = total_parts;
+    total_parts += nparts[bg];
+    if (nparts[bg] > 512 || nparts[bg] < 1) return SEKV_OK;                               // combine capacity: generic path
+  }
+  part_base[BG] = total_parts;
+  if ((int)items.size() > F.max_items || total_parts > F.max_chunks) return SEKV_OK;
+  h->n_items = (int)items.size();
+  CK(h, cudaMemcpyAsync(h->dev + F.off_items_sched, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_part, part_base.data(), part_base.size() * 4, cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_route, route_items.data(), route_items.size() * 4, cudaMemcpyHostToDevice, h->main));
+  CK(h, cudaStreamSynchronize(h->main));
+  h->use_fused = true;
+  return SEKV_OK;
+}
+
 static sekv_status ensure_segmented(sekv_handle* h, int n_seqs, const int64_t* seq_tok_off, const float* H) {
   const sekv_config& c = h->cfg;
   if (n_seqs < 1 || n_seqs > c.max_seqs) return fail(h, SEKV_INVALID_ARG, "n_seqs out of range");
@@ -389,7 +484,9 @@ static sekv_status ensure_segmented(sekv_handle* h, int n_seqs, const int64_t* s
   h->m_tot = 0; h->A_tot = 0; h->max_m = 0;
   for (int b = 0; b < n_seqs; ++b) { h->m_tot += m[b]; h->A_tot += a[b]; h->max_m = std::max(h->max_m, m[b]); }
   h->segmented = true;
-  return make_schedule(h);
+  sekv_status ss = make_schedule(h);
+  if (ss != SEKV_OK) return ss;
+  return make_fused_schedule(h);
 }
 
 static sekv_status assign_blobs(sekv_handle* h, int layer, const std::vector<int32_t>& rk, const std::vector<int32_t>& rv) {
@@ -537,7 +634,13 @@ sekv_status sekv_route(sekv_handle* h, int32_t layer, const void* q, const float
   if (!q || !ids || !count) return fail(h, SEKV_INVALID_ARG, "q, ids or count is NULL");
   if ((s = check_k(h, k)) != SEKV_OK) return s;
   cudaError_t e;
-  { ProfScope ps(h, 0, h->main); e = launch_route(h, layer, q, tau, k, logits, alpha_tilde, ids, count, h->main); }
+  if (h->use_fused) {
+    ProfScope ps(h, 6, h->main);
+    e = launch_fused(h, layer, FM_ROUTE, q, tau, k, logits, alpha_tilde, ids, count, nullptr, nullptr, h->main);
+  } else {
+    ProfScope ps(h, 0, h->main);
+    e = launch_route(h, layer, q, tau, k, logits, alpha_tilde, ids, count, h->main);
+  }
   if (e != cudaSuccess) return cuda_fail(h, e, "route");
   return SEKV_OK;
 }
@@ -545,6 +648,10 @@ sekv_status sekv_route(sekv_handle* h, int32_t layer, const void* q, const float
 static cudaError_t decode_layer(sekv_handle* h, int layer, const void* q, const int32_t* ids, const int32_t* count,
                                 void* out, float* lse) {
   cudaError_t e;
+  if (h->use_fused) {     // caller-supplied zoom set: plan + attention + combine in the fused layer kernel
+    ProfScope ps(h, 6, h->main);
+    return launch_fused(h, layer, FM_ATTN, q, nullptr, 0, nullptr, nullptr, (int32_t*)ids, (int32_t*)count, out, lse, h->main);
+  }
   { ProfScope ps(h, 1, h->main); if ((e = launch_plan(h, layer, ids, count, h->main)) != cudaSuccess) return e; }
   if (h->cfg.k_cap > 0) {
     if ((e = cudaEventRecord(h->ev_fork, h->main)) != cudaSuccess) return e;
@@ -580,18 +687,47 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
   const size_t qstride = (size_t)B * c.n_q_heads * kD * h->esize;
   const size_t ostride = (size_t)B * c.n_q_heads * kD * (c.out_dtype == SEKV_BF16 ? 2 : 4);
   const int kcap = std::max(c.k_cap, 1);
+  bool forked = false;
   for (int l = 0; l < c.n_layers; ++l) {
     const uint8_t* ql = (const uint8_t*)q + l * qstride;
     int32_t* ids = (int32_t*)(h->dev + h->F.off_ws_ids) + (size_t)l * c.max_seqs * c.n_kv_heads * kcap;
     int32_t* cnt = (int32_t*)(h->dev + h->F.off_ws_count) + (size_t)l * c.max_seqs * c.n_kv_heads;
     cudaError_t e;
+    void* ol = (uint8_t*)out + l * ostride;
+    float* ll = lse ? lse + (size_t)l * B * c.n_q_heads : nullptr;
+    if (h->use_fused) {
+      {
+        ProfScope ps(h, 6, h->main);
+        if (c.k_cap > 0)
+          e = launch_fused(h, l, FM_ROUTE | FM_ATTN, ql, tau ? tau + (size_t)l * c.n_q_heads : nullptr, k, nullptr,
+                           nullptr, ids, cnt, ol, ll, h->main);
+        else
+          e = launch_fused(h, l, FM_ATTN, ql, nullptr, 0, nullptr, nullptr, nullptr, nullptr, ol, ll, h->main);
+      }
+      if (e != cudaSuccess) return e;
+      if (c.k_cap > 0 && c.prefetch > 0 && k >= 0) {
+        // speculative prefetch of the next-best spans of this layer on the side stream; it overlaps the
+        // following layers and is joined at the end of the step (this layer's cache is next read one step later)
+        if ((e = cudaEventRecord(h->ev_fork, h->main)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(h->side, h->ev_fork, 0)) != cudaSuccess) return e;
+        ProfScope ps(h, 7, h->side);
+        if ((e = launch_prefetch(h, l, h->side)) != cudaSuccess) return e;
+        forked = true;
+      }
+      continue;
+    }
     if (c.k_cap > 0) {
       ProfScope ps(h, 0, h->main);
       e = launch_route(h, l, ql, tau ? tau + (size_t)l * c.n_q_heads : nullptr, k, nullptr, nullptr, ids, cnt, h->main);
       if (e != cudaSuccess) return e;
     }
-    e = decode_layer(h, l, ql, ids, cnt, (uint8_t*)out + l * ostride, lse ? lse + (size_t)l * B * c.n_q_heads : nullptr);
+    e = decode_layer(h, l, ql, ids, cnt, ol, ll);
     if (e != cudaSuccess) return e;
+  }
+  if (forked) {
+    cudaError_t e;
+    if ((e = cudaEventRecord(h->ev_join, h->side)) != cudaSuccess) return e;
+    if ((e = cudaStreamWaitEvent(h->main, h->ev_join, 0)) != cudaSuccess) return e;
   }
   return cudaSuccess;
 }
@@ -639,6 +775,20 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   return SEKV_OK;
 }
 
+sekv_status sekv_last_zoom_ids(sekv_handle* h, int32_t layer, int32_t* ids, int32_t* count) {
+  if (!h) return SEKV_INVALID_ARG;
+  sekv_status s = check_ready(h, layer);
+  if (s != SEKV_OK) return s;
+  if (!ids || !count) return fail(h, SEKV_INVALID_ARG, "ids or count is NULL");
+  const sekv_config& c = h->cfg;
+  const int kcap = std::max(c.k_cap, 1);
+  const int32_t* wi = (const int32_t*)(h->dev + h->F.off_ws_ids) + (size_t)layer * c.max_seqs * c.n_kv_heads * kcap;
+  const int32_t* wc = (const int32_t*)(h->dev + h->F.off_ws_count) + (size_t)layer * c.max_seqs * c.n_kv_heads;
+  CK(h, cudaMemcpyAsync(ids, wi, (size_t)h->n_seqs * c.n_kv_heads * kcap * 4, cudaMemcpyDeviceToDevice, h->main));
+  CK(h, cudaMemcpyAsync(count, wc, (size_t)h->n_seqs * c.n_kv_heads * 4, cudaMemcpyDeviceToDevice, h->main));
+  return SEKV_OK;
+}
+
 sekv_status sekv_decode_step_host(sekv_handle* h, const void* q_host, const float* tau, int32_t k, void* out_host,
                                   float* lse_host) {
   if (!h) return SEKV_INVALID_ARG;
@@ -679,6 +829,7 @@ sekv_status sekv_get_stats(sekv_handle* h, sekv_stats* out) {
   out->h2d_bytes = v[ST_H2D];
   out->factor_bytes_algo = v[ST_FACTOR_ALGO];
   out->coarse_rows_skipped = v[ST_SKIPPED];
+  out->prefetched_spans = v[ST_PREFETCHED];
   out->kernel_launches = h->launches;
   return SEKV_OK;
 }

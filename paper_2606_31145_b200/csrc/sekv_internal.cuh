@@ -22,12 +22,14 @@ constexpr int kStage2SpansPerCta = 4;
 __host__ __device__ inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 __host__ __device__ inline size_t round_up_sz(size_t x, size_t m) { return (x + m - 1) / m * m; }
 
-// ---- factor blob layout (DESIGN.md section 6) ------------------------------------------------
-// [sigma_K f32 rkp][sigma_V f32 rvp][VtK st rkp x 128][VV st 128 x rvp][UK st lenp x rkp][UVt st rvp x lenp]
-// Each operand is stored with its contraction index contiguous.
+// ---- factor blob layout (DESIGN.md section 5) ------------------------------------------------
+// header : [sigma_K f32 rkp][sigma_V f32 rvp][VtK st rkp x 128][VV st 128 x rvp]
+// chunks : lenp/16 chunks of 16 tokens, each [UK st 16 x rkp][UVt st rvp x 16]
+// Each operand is stored with its contraction index contiguous; a chunk is one contiguous piece, so a
+// whole blob (or any run of chunks) moves with a single 1-D bulk copy (cp.async.bulk).
 struct BlobDims {
   int len, lenp, rk, rv, rkp, rvp;
-  size_t off_sk, off_sv, off_vtk, off_vv, off_uk, off_uvt, bytes;
+  size_t off_sk, off_sv, off_vtk, off_vv, off_chunks, chunk_bytes, uvt_in_chunk, bytes;
 };
 __host__ __device__ inline BlobDims blob_dims(int esize, int len, int rk, int rv) {
   BlobDims b;
@@ -40,10 +42,19 @@ __host__ __device__ inline BlobDims blob_dims(int esize, int len, int rk, int rv
   b.off_sv = o;  o += (size_t)b.rvp * 4;
   b.off_vtk = o; o += (size_t)b.rkp * kD * esize;
   b.off_vv = o;  o += (size_t)kD * b.rvp * esize;
-  b.off_uk = o;  o += (size_t)b.lenp * b.rkp * esize;
-  b.off_uvt = o; o += (size_t)b.rvp * b.lenp * esize;
+  b.off_chunks = o;
+  b.uvt_in_chunk = (size_t)kLenPad * b.rkp * esize;
+  b.chunk_bytes = (size_t)kLenPad * (b.rkp + b.rvp) * esize;
+  o += (size_t)(b.lenp / kLenPad) * b.chunk_bytes;
   b.bytes = round_up_sz(o, 128);
   return b;
+}
+// byte offset of U_K[t][i] and of U_V[t][i] (stored transposed inside the chunk) within a blob
+__host__ __device__ inline size_t blob_uk_off(const BlobDims& b, int esize, int t, int i) {
+  return b.off_chunks + (size_t)(t / kLenPad) * b.chunk_bytes + ((size_t)(t % kLenPad) * b.rkp + i) * esize;
+}
+__host__ __device__ inline size_t blob_uv_off(const BlobDims& b, int esize, int t, int i) {
+  return b.off_chunks + (size_t)(t / kLenPad) * b.chunk_bytes + b.uvt_in_chunk + ((size_t)i * kLenPad + (t % kLenPad)) * esize;
 }
 
 // ---- device views ------------------------------------------------------------------------------
@@ -70,8 +81,8 @@ struct LayerView {
   uint8_t* slots;          // [B][H_kv][ways][slot_bytes]
   uint32_t* layer_step;    // [1]
   uint32_t* zoom_mask;     // [B][H_kv][mask_words]
-  uint32_t* items;         // [B][H_kv][k_cap]  way | miss << 31, valid for j < count
-  int32_t* item_span;      // [B][H_kv][k_cap]  local span id (deduplicated; -1 = dropped)
+  uint32_t* items;         // [B][H_kv][kc]  way | miss << 31, valid for j < count (kc = max(k_cap,1) + prefetch)
+  int32_t* item_span;      // [B][H_kv][kc]  local span id (deduplicated; -1 = dropped)
 };
 
 struct Dims {
@@ -89,7 +100,44 @@ struct Chunk {  // one stage-1 work item
   int32_t part;       // partial slot within the head
 };
 
-enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_COUNT = 8 };
+enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_PREFETCHED, ST_COUNT = 8 };
+
+// ---- fused layer kernel (fused_kernels.cu) -------------------------------------------------------
+enum ItemKind { IT_ROUTE = 0, IT_POOL = 1, IT_ZOOM = 2, IT_COARSE = 3 };
+enum FusedMode { FM_ROUTE = 1, FM_ATTN = 2 };   // FM_ATTN without FM_ROUTE: caller-supplied zoom set
+struct Item {          // one work item of the layer kernel's queue
+  int32_t kind;        // ItemKind
+  int32_t bg;          // b * H_kv + g
+  int32_t a, b;        // ROUTE: span range; POOL / COARSE: entry-row range; ZOOM: plan-item range
+  int32_t part;        // partial slot within the group (attention items)
+};
+
+struct FusedParams {
+  CsrView cv;
+  LayerView lv;
+  const __nv_bfloat16* q;      // [B][H][128]
+  const float* tau;            // [H] or null
+  float* logits_out;           // [H][m_tot] or null
+  float* alpha_out;
+  int32_t* ids;                // [B][H_kv][k_cap]: written (FM_ROUTE) or read (caller-supplied zoom set)
+  int32_t* count;              // [B][H_kv]
+  void* out;                   // [B][H][128]
+  float* lse;                  // [B][H] or null
+  const Item* items;
+  const int32_t* bg_part_base;   // [BG+1] first partial of each group
+  const int32_t* bg_route_items; // [BG]   route chunk items per group
+  float* partials;
+  unsigned long long* keys;    // [BG][sort_n]
+  int32_t* ctrs;               // [0] queue, [1] exited CTAs, then per group: route_done, attn_done, plan_flag
+  int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
+  unsigned long long* stats;
+  const uint8_t* host_arena;   // device alias of the pinned host factor store
+  size_t ent_head_stride, route_head_stride;
+  int64_t slot_bytes, smem_buf_stride;
+  int32_t n_items, mode, k, k_cap, prefetch, kc;
+  int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, sort_n, out_bf16;
+  int32_t sm_ids, sm_wayof, sm_tags, sm_mask;   // byte offsets in dynamic shared memory (plan)
+};
 
 // ---- storage-type helpers ------------------------------------------------------------------------
 template <typename ST> struct StTraits;
@@ -144,8 +192,9 @@ struct FullLayout {
   sekv_layout lay;
   int64_t off_partials1, off_partials2, off_ws_ids, off_ws_count, off_stats, off_chunks, off_bg_chunk,
       off_zoom_mask, off_items, off_item_span, off_layer_step, off_seg_flag, off_seg_flag2, off_seg_len,
-      off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag;
-  int mask_words, max_chunks;
+      off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag, off_items_sched, off_bg_part,
+      off_bg_route, off_keys, off_ctrs, off_plan_counts;
+  int mask_words, max_chunks, max_items, ctrs_per_layer, keys_per_bg;
   size_t total;
 };
 
@@ -172,6 +221,9 @@ struct sekv_handle {
   size_t host_used;
   // schedule
   int n_chunks, parts1_max, P2, parts_per_head, sort_n;
+  // fused layer kernel (bf16 path)
+  bool use_fused;
+  int n_items, n_route_items, fused_grid, fused_occ, fused_item_rows;
   int num_sms;
   std::vector<GraphEntry> graphs;
   uint64_t launches;
@@ -212,6 +264,11 @@ cudaError_t launch_fetch(sekv_handle* h, int layer, const int32_t* count, cudaSt
 cudaError_t launch_stage1(sekv_handle* h, int layer, const void* q, cudaStream_t s);
 cudaError_t launch_stage2(sekv_handle* h, int layer, const void* q, const int32_t* count, cudaStream_t s);
 cudaError_t launch_combine(sekv_handle* h, int layer, void* out, float* lse, cudaStream_t s);
+cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
+                         float* alpha, int32_t* ids, int32_t* count, void* out, float* lse, cudaStream_t s);
+cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s);
+size_t fused_smem_bytes(const sekv_handle* h, FusedParams* P);
+int fused_occupancy(const sekv_handle* h);
 
 inline uint8_t* ws(const sekv_handle* h, int64_t off) { return h->dev + off; }
 

@@ -13,7 +13,8 @@ from . import binding as B
 
 def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Optional[int] = None,
                out_dtype: str = "f32", use_graph: int = 0, impl: int = 0, stage1_ctas: int = 0,
-               r_max: Optional[int] = None, slack: float = 1.0) -> B.sekv_config:
+               r_max: Optional[int] = None, slack: float = 1.0, prefetch: int = 0, item_rows: int = 0,
+               zoom_spans_per_item: int = 0) -> B.sekv_config:
     m_tot = sum(l.m for l in layouts)
     a_tot = sum(l.A for l in layouts)
     n_tot = sum(l.n for l in layouts)
@@ -21,8 +22,10 @@ def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Option
     max_len = max(int(l.planted_span_len.max()) if l.m else 1 for l in layouts)
     if k_cap is None:
         k_cap = max_m if spec.top_k < 0 else spec.top_k
+    if spec.top_k < 0:
+        prefetch = 0
     if cache_ways is None:
-        cache_ways = max(2 * k_cap, 1) if spec.top_k >= 0 else max(k_cap, 1)
+        cache_ways = max(2 * (k_cap + prefetch), 1) if spec.top_k >= 0 else max(k_cap, 1)
     return B.make_config(
         n_layers=spec.n_layers, n_q_heads=spec.n_q_heads, n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim,
         route_dim=spec.route_dim, dtype=B.SEKV_BF16 if spec.dtype == "bf16" else B.SEKV_F32,
@@ -30,7 +33,8 @@ def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Option
         r_max=r_max or spec.rank, window=spec.window, max_seqs=len(layouts), max_tokens_total=n_tot,
         max_spans_total=int(m_tot * slack) + 1, max_full_total=int(a_tot * slack) + 1,
         max_span_len=min(1024, -(-max(max_len, 16) // 16) * 16), k_cap=k_cap, cache_ways=max(cache_ways, 1),
-        stage1_ctas=stage1_ctas, use_graph=use_graph, impl=impl)
+        prefetch=prefetch, stage1_ctas=stage1_ctas, item_rows=item_rows, zoom_spans_per_item=zoom_spans_per_item,
+        use_graph=use_graph, impl=impl)
 
 
 def host_bytes_for(spec, layouts, cfg: B.sekv_config) -> int:

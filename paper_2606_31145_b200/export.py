@@ -20,7 +20,9 @@ def _f64(t: torch.Tensor) -> np.ndarray:
 
 
 def blob_sections(esize: int, ln: int, rk: int, rv: int) -> dict:
-    """Byte offsets of a factor blob; mirrors the layout stated in sekv.h."""
+    """Byte offsets of a factor blob; mirrors the layout stated in sekv_internal.cuh:
+    header [sK f32 rkp][sV f32 rvp][VtK rkp x 128][VV 128 x rvp], then lenp/16 chunks of 16 tokens,
+    each [UK 16 x rkp][UVt rvp x 16]."""
     lenp = -(-ln // 16) * 16
     rkp = -(-max(rk, 1) // 8) * 8
     rvp = -(-max(rv, 1) // 8) * 8
@@ -30,8 +32,7 @@ def blob_sections(esize: int, ln: int, rk: int, rv: int) -> dict:
     sec["sv"] = o; o += rvp * 4
     sec["vtk"] = o; o += rkp * 128 * esize
     sec["vv"] = o; o += 128 * rvp * esize
-    sec["uk"] = o; o += lenp * rkp * esize
-    sec["uvt"] = o; o += rvp * lenp * esize
+    sec["chunks"] = o; o += lenp * (rkp + rvp) * esize
     sec["bytes"] = -(-o // 128) * 128
     return sec
 
@@ -86,8 +87,10 @@ def export_tables(eng: B.Sekv, layer: int, b: int, with_factors: bool = True) ->
                 sV = blob[sec["sv"]:sec["sv"] + sec["rvp"] * 4].view(torch.float32)
                 VtK = blob[sec["vtk"]:sec["vtk"] + sec["rkp"] * 128 * es].view(st).view(sec["rkp"], 128)
                 VV = blob[sec["vv"]:sec["vv"] + 128 * sec["rvp"] * es].view(st).view(128, sec["rvp"])
-                UK = blob[sec["uk"]:sec["uk"] + sec["lenp"] * sec["rkp"] * es].view(st).view(sec["lenp"], sec["rkp"])
-                UVt = blob[sec["uvt"]:sec["uvt"] + sec["rvp"] * sec["lenp"] * es].view(st).view(sec["rvp"], sec["lenp"])
+                ch = blob[sec["chunks"]:sec["chunks"] + sec["lenp"] * (sec["rkp"] + sec["rvp"]) * es].view(st)
+                ch = ch.view(sec["lenp"] // 16, 16 * (sec["rkp"] + sec["rvp"]))
+                UK = ch[:, :16 * sec["rkp"]].reshape(sec["lenp"], sec["rkp"])                       # [lenp][rkp]
+                UVt = ch[:, 16 * sec["rkp"]:].reshape(sec["lenp"] // 16, sec["rvp"], 16).permute(1, 0, 2).reshape(sec["rvp"], sec["lenp"])
                 row.append(dict(UK=_f64(UK[:ln, :rk]), sK=_f64(sK[:rk]), VtK=_f64(VtK[:rk]),
                                 UV=_f64(UVt[:rv, :ln]).T.copy(), sV=_f64(sV[:rv]), VtV=_f64(VV[:, :rv]).T.copy(),
                                 pad_ok=bool((UK[ln:].float() == 0).all() and (UVt[:, ln:].float() == 0).all()

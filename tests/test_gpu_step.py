@@ -1,0 +1,103 @@
+"""GPU parity of the whole-step entry point (sekv_decode_step): routing, residency plan, demand fetch,
+side-stream prefetch, mixed-resolution attention and combine in ONE call per step, over several steps of an
+AR(1) query stream so that the device factor cache goes through misses, hits, evictions and prefetches.
+Every step's zoom sets and outputs are compared with the oracle on the exported tables."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import sekv_oracle as O
+from tests.gpu_common import TOL_BF16, tables_from_export
+from tests.helpers import check_ids, rel_l2, to_np
+from workloads import get_spec, make_layer_inputs, make_layouts, make_queries, next_queries_ar1
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_steps(spec, n_steps, rho, heads=None, **cfg_kw):
+    from paper_2606_31145_b200 import engine as E
+    from paper_2606_31145_b200.export import export_tables
+    lay = make_layouts(spec)
+    eng = E.create_engine(spec, lay, **cfg_kw)
+    tabs = [[tables_from_export(export_tables(eng, l, b), spec.n_q_heads, spec.n_kv_heads, spec.route_dim)
+             for b in range(eng.n_seqs)] for l in range(spec.n_layers)]
+    L, B, Hq, Hkv = spec.n_layers, spec.batch, spec.n_q_heads, spec.n_kv_heads
+    q = make_queries(spec, 0, "cuda")
+    out = torch.zeros((L, B, Hq, 128), dtype=torch.float32, device="cuda")
+    lse = torch.zeros((L, B, Hq), dtype=torch.float32, device="cuda")
+    hs = list(range(Hq)) if heads is None else list(heads)
+    worst = dict(rel_l2=0.0, max_abs=0.0, lse=0.0)
+    for step in range(n_steps):
+        eng.sekv_decode_step(q, spec.top_k, out, lse=lse)
+        torch.cuda.synchronize()
+        out_h = out.cpu().numpy().astype(np.float64)
+        lse_h = lse.cpu().numpy().astype(np.float64)
+        qn = to_np(q)
+        for l in range(L):
+            ids, count = eng.sekv_last_zoom_ids(l)
+            torch.cuda.synchronize()
+            ids_h, count_h = ids.cpu().numpy(), count.cpu().numpy()
+            for b in range(B):
+                T = tabs[l][b]
+                R = O.route(qn[l, b], T.W, T.route_K, T.seg.span_len, Hkv, spec.top_k)
+                zoom = []
+                for g in range(Hkv):
+                    c = int(count_h[b, g])
+                    assert c == len(R.ids[g])
+                    check_ids(ids_h[b, g, :c], R.ids[g], R.group_logit[g])
+                    zoom.append([int(x) for x in ids_h[b, g, :c]])
+                ref, ref_lse = O.decode_attn(qn[l, b], T, zoom, heads=hs)
+                r = rel_l2(out_h[l, b, hs], ref[hs])
+                a = float(np.abs(out_h[l, b, hs] - ref[hs]).max())
+                e = float(np.abs(lse_h[l, b, hs] - ref_lse[hs]).max())
+                worst = dict(rel_l2=max(worst["rel_l2"], r), max_abs=max(worst["max_abs"], a), lse=max(worst["lse"], e))
+                assert r <= TOL_BF16["rel_l2"] and a <= TOL_BF16["max_abs"] and e <= TOL_BF16["lse"], (step, l, b, r, a, e)
+        q = next_queries_ar1(spec, q, step + 1, rho)
+    st = eng.sekv_get_stats()
+    return eng, st, worst
+
+
+@pytest.mark.parametrize("prefetch", [0, 8])
+def test_step_config1_sharp_two_layers(prefetch):
+    spec = get_spec(1).sharp().with_(n_layers=2, contexts=(20000,))
+    eng, st, worst = _run_steps(spec, 5, 0.7, prefetch=prefetch)
+    print("step cfg1", prefetch, worst, st)
+    assert st["zoomed_spans"] == 5 * 2 * 8 * 16 == st["cache_hits"] + st["cache_misses"]
+    assert st["layer_steps"] == 10
+    assert st["cache_misses"] >= 2 * 8 * 16            # cold start
+    assert st["cache_hits"] > 0                         # later steps reuse cached factors
+    if prefetch:
+        assert st["prefetched_spans"] > 0
+    else:
+        assert st["prefetched_spans"] == 0
+    eng.close()
+
+
+def test_step_prefetch_reduces_demand_misses():
+    """Same stream with and without the speculative prefetch: identical outputs (checked against the oracle in
+    both runs), fewer demand misses with it."""
+    spec = get_spec(1).sharp().with_(contexts=(24000,))
+    eng0, st0, _ = _run_steps(spec, 6, 0.9, heads=[0, 9, 31], prefetch=0, cache_ways=64)
+    eng0.close()
+    eng1, st1, _ = _run_steps(spec, 6, 0.9, heads=[0, 9, 31], prefetch=16, cache_ways=64)
+    eng1.close()
+    assert st1["cache_misses"] < st0["cache_misses"], (st0, st1)
+
+
+def test_step_ragged_batch_graph_replay():
+    """Ragged batch (config 3, B = 3) through the CUDA-graph path: replays must see the new queries."""
+    spec = get_spec(3, batch=3)
+    eng, st, worst = _run_steps(spec, 3, 0.9, heads=[0, 13, 31], prefetch=4, use_graph=1)
+    print("step cfg3", worst)
+    assert st["layer_steps"] == 3
+    eng.close()
+
+
+def test_step_small_cache_evicts_lru():
+    """cache_ways == k_cap + prefetch: every miss evicts; results stay exact."""
+    spec = get_spec(1).sharp().with_(contexts=(16000,))
+    eng, st, _ = _run_steps(spec, 4, 0.3, heads=[1, 18], prefetch=2, cache_ways=18)
+    assert st["cache_misses"] > 8 * 16
+    eng.close()
