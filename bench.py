@@ -40,6 +40,10 @@ def parse():
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--generic", action="store_true", help="force the generic (non tensor-core) kernels")
     ap.add_argument("--stage1-ctas", type=int, default=0)
+    ap.add_argument("--prefetch", type=int, default=8, help="speculative prefetch depth per (sequence, kv head)")
+    ap.add_argument("--cache-ways", type=int, default=0)
+    ap.add_argument("--item-rows", type=int, default=0)
+    ap.add_argument("--zoom-spans", type=int, default=0)
     ap.add_argument("--profile-steps", type=int, default=4)
     ap.add_argument("--e2e-steps", type=int, default=8)
     return ap.parse_args()
@@ -184,7 +188,9 @@ def run_ours(args):
     layouts = make_layouts(spec)
     t_setup = time.time()
     cfg = E.config_for(spec, layouts, out_dtype="bf16", use_graph=0 if args.no_graph else 1,
-                       impl=1 if args.generic else 0, stage1_ctas=args.stage1_ctas)
+                       impl=1 if args.generic else 0, stage1_ctas=args.stage1_ctas, prefetch=args.prefetch,
+                       cache_ways=args.cache_ways or None, item_rows=args.item_rows,
+                       zoom_spans_per_item=args.zoom_spans)
     eng = B.Sekv(cfg, E.host_bytes_for(spec, layouts, cfg), device=dev)
     H_dev = E.surprisal_device(layouts, eng.device)
     for layer in range(spec.n_layers):
@@ -255,19 +261,26 @@ def run_ours(args):
     kt = eng.sekv_get_kernel_times()
     st_p = eng.sekv_get_stats()
     eng.sekv_set_profiling(False)
-    tot_kernel_ms = sum(v["ms"] for k, v in kt.items() if k != "fetch")
-    s1 = kt["stage1"]
-    s1_us = s1["ms"] * 1e3 / max(1, s1["launches"])
-    # algorithmic bytes of one stage-1 launch: pool + unexpanded coarse rows (K and V) + q + out partials excluded
-    rows_bytes = sum(2 * spec.n_kv_heads * (a + m) * 128 * esz for a, m in zip(eng.pool_per_seq, eng.spans_per_seq))
-    s1_bytes = rows_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz / max(1, s1["launches"]) + Bn * Hq * 128 * esz
+    tot_kernel_ms = sum(v["ms"] for k, v in kt.items() if k not in ("fetch", "prefetch"))
     peak, peak_src = measured_peaks()
-    roofline = {"bound": "hbm", "kernel": "stage1_mma_kernel (a5: pool + coarse entries)" if not args.generic else "stage1_kernel",
-                "achieved": s1_bytes / (s1_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
-                "frac": s1_bytes / (s1_us * 1e-6) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": s1_bytes, "avg_launch_us": s1_us,
-                "share_of_step_kernel_time": s1["ms"] / max(1e-9, tot_kernel_ms),
-                "kernel_us_per_layer": {k: v["ms"] * 1e3 / max(1, v["launches"]) for k, v in kt.items()}}
+    prof_layer_steps = max(1, st_p["layer_steps"])
+    if kt["fused"]["launches"]:
+        # ONE kernel per layer-step does a1-a7: its algorithmic bytes are the layer-step's
+        dom, dom_name = kt["fused"], "fused_layer_kernel (a1-a7: route, plan, pool/coarse/zoom partials, combine)"
+        dom_bytes = (prof_layer_steps * static_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz
+                     + st_p["factor_bytes_algo"]) / prof_layer_steps
+    else:
+        dom, dom_name = kt["stage1"], "stage1 kernel (a5: pool + coarse entries)"
+        rows_bytes = sum(2 * spec.n_kv_heads * (a + m) * 128 * esz for a, m in zip(eng.pool_per_seq, eng.spans_per_seq))
+        dom_bytes = rows_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz / prof_layer_steps + Bn * Hq * 128 * esz
+    dom_us = dom["ms"] * 1e3 / max(1, dom["launches"])
+    roofline = {"bound": "hbm", "kernel": dom_name,
+                "achieved": dom_bytes / (dom_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_us": dom_us,
+                "share_of_step_kernel_time": dom["ms"] / max(1e-9, tot_kernel_ms),
+                "timing": "CUDA events on the launching stream around every launch, eager launches, %d steps" % args.profile_steps,
+                "kernel_us_per_launch": {k: v["ms"] * 1e3 / v["launches"] for k, v in kt.items() if v["launches"]}}
 
     # ---- end to end through host buffers -----------------------------------------------------------------
     q_host = [q_all[qi + i].cpu().pin_memory() for i in range(args.e2e_steps)]
@@ -307,7 +320,8 @@ def run_ours(args):
                    "kv_heads": spec.n_kv_heads, "rank": spec.rank, "top_k": spec.top_k, "rho": args.rho,
                    "spans_per_seq": eng.spans_per_seq, "pool_per_seq": eng.pool_per_seq,
                    "cache_ways": cfg.cache_ways, "cache_hit_rate": hit, "graph": not args.no_graph,
-                   "kernels": "generic" if args.generic else "mma.sync bf16", "stage1_ctas": n_ctas,
+                   "kernels": "generic multi-kernel" if args.generic else "fused persistent layer kernel (mma.sync bf16, TMA bulk factor copies)",
+                   "prefetch": cfg.prefetch, "stage1_ctas": n_ctas,
                    "l2": "inputs larger than L2: one step streams %.2f GB of tables (L2 = 126 MB), no flush" % (algo_bytes / args.steps / 1e9),
                    "replicas": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
                    "setup_s": round(t_setup, 1)},
