@@ -273,7 +273,7 @@ def run_ours(args):
         dom, dom_name = kt["stage1"], "stage1 kernel (a5: pool + coarse entries)"
         rows_bytes = sum(2 * spec.n_kv_heads * (a + m) * 128 * esz for a, m in zip(eng.pool_per_seq, eng.spans_per_seq))
         dom_bytes = rows_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz / prof_layer_steps + Bn * Hq * 128 * esz
-    dom_us = dom["ms"] * 1e3 / max(1, dom["launches"])
+    dom_us = max(dom["ms"] * 1e3 / max(1, dom["launches"]), 1e-9)
     roofline = {"bound": "hbm", "kernel": dom_name,
                 "achieved": dom_bytes / (dom_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
                 "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak, "traffic": None, "peak_source": peak_src,

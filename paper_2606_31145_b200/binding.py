@@ -97,12 +97,13 @@ def _load() -> C.CDLL:
     lib.sekv_get_schedule.argtypes = [VP, P(I32), P(I32)]
     lib.sekv_set_profiling.argtypes = [VP, I32]
     lib.sekv_get_kernel_times.argtypes = [VP, P(C.c_double), P(C.c_uint64)]
+    lib.sekv_set_trace.argtypes = [VP, VP, I64, P(I32)]
     for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
                  "sekv_last_zoom_ids",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
                  "sekv_static_bytes_per_layer", "sekv_get_schedule", "sekv_set_profiling",
-                 "sekv_get_kernel_times"):
+                 "sekv_get_kernel_times", "sekv_set_trace"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -322,6 +323,14 @@ class Sekv:
         ms, n = (C.c_double * 8)(), (C.c_uint64 * 8)()
         self._check(lib.sekv_get_kernel_times(self._h, ms, n), "sekv_get_kernel_times")
         return {name: dict(ms=float(ms[i]), launches=int(n[i])) for i, name in enumerate(self.KERNEL_CLASSES)}
+
+    def sekv_set_trace(self, buf: Optional[torch.Tensor]) -> int:
+        """buf: uint8/int64 DEVICE tensor of 64 bytes per item, or None to switch tracing off."""
+        n = C.c_int32(0)
+        cap = 0 if buf is None else buf.numel() * buf.element_size() // 64
+        self._check(lib.sekv_set_trace(self._h, _ptr(buf), cap, C.byref(n)), "sekv_set_trace")
+        self._trace_buf = buf
+        return int(n.value)
 
     def sekv_get_schedule(self):
         a, b = C.c_int32(0), C.c_int32(0)

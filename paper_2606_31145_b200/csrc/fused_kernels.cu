@@ -1,25 +1,30 @@
 // The bf16 hot path: ONE persistent kernel per layer-step that runs a1-a7 (Eq. 4, 5, 9, L123,
-// L119-121, Eq. 8) as work items pulled from a dependency-ordered queue:
+// L119-121, Eq. 8).  One CTA per SM; every WARP is an independent worker with a private shared-memory
+// region and pulls work items from two dependency-ordered queues (first item static, then atomic claims
+// two items ahead so neither the claim nor the descriptor load is on the warp's critical path):
 //
-//   ROUTE  (b, g, span chunk)   q' = W q, x = q'.K_bar/sqrt(d') + ln|S|, alpha = sig(x), X = max over the
-//                               group, 64-bit keys -> global.  The LAST chunk of a (b, g) to finish sorts
-//                               the keys (top-k, ties to the lower id), runs the residency plan of the
-//                               device factor cache (LRU) and releases plan_flag[b, g].
-//   POOL   (b, g, row range)    online-softmax partial over full-resolution tokens (no dependency).
-//   ZOOM   (b, g, item range)   expanded spans through the factored form: the span's factor blob is moved
-//                               by ONE 1-D bulk async copy (TMA engine) into shared memory -- from its cache
-//                               slot on a hit, straight from the pinned-host store over PCIe on a demand
-//                               miss (and then written to the slot) -- double-buffered across spans.
-//   COARSE (b, g, row range)    partial over the unexpanded coarse entries (+ln|S|); needs the zoom mask.
+//   latency queue (even warps start here)
+//     QPROJ   (b, h)              q' = W q (Eq. 4): coalesced 16-byte loads of W, half-warp shuffle reduction
+//     ROUTE   (b, g, 64 spans)    x = q'.K_bar/sqrt(d') + ln|S|, alpha = sig(x) (Eq. 5), X = max over the group
+//                                 (GQA), ordered 32-bit keys -> global
+//     SELECT  (b, g)              top-k (Eq. 9, cap L123) by a 4-pass radix select on the keys, ties to the lower
+//                                 span id, sorted ids; then the residency plan of the device factor cache (LRU),
+//                                 zoom bit-mask, one descriptor per expanded span
+//   main queue
+//     POOL    (b, g, row range)   online-softmax partial over full-resolution tokens (no dependency): K/V rows
+//                                 stream through a 3-stage cp.async ring (XOR-swizzled, bank-conflict free)
+//     ZOOM    (b, g, plan items)  expanded spans through the factored form; the span's factor blob moves by ONE
+//                                 1-D bulk async copy (TMA engine) into the warp's region -- from its cache slot
+//                                 on a hit, straight from the pinned-host store over PCIe on a demand miss (and is
+//                                 then written to the slot)
+//     COARSE  (b, g, row range)   partial over the unexpanded coarse entries (+ln|S|); needs the zoom mask
+//     COMBINE (b, h)              log-sum-exp merge of the head's partials -> output (a7)
 //
-// ZOOM and COARSE items wait on plan_flag[b, g]; the queue order (ROUTE, POOL..., ZOOM, COARSE) is a
-// topological order and items are claimed in queue order, so a waiting CTA only ever waits on work that
-// a running CTA has already claimed: no co-residency assumption, no deadlock.  The LAST attention item of
-// a (b, g) to finish merges that group's partials by log-sum-exp and writes the output (a7).
+// Waiting items only ever wait on items earlier in their queue (or in the latency queue), claims are in
+// queue order and the grid is resident (one CTA per SM), so the wait graph is acyclic.
 //
 // Tensor cores: G <= 8 query heads per kv head is far below a tcgen05 tile and the path is HBM-bound, so
-// the heads are the (padded) 16 rows of warp-level mma.sync.m16n8k16 tiles; K/V rows stream from global
-// memory straight into B fragments (every byte read once, coalesced 16-byte loads).
+// the heads are the (padded) 16 rows of warp-level mma.sync.m16n8k16 tiles.
 #include <algorithm>
 
 #include "mma_common.cuh"
@@ -28,9 +33,8 @@ namespace sekv {
 
 namespace {
 
-constexpr int kFT = 128;        // threads per CTA
-constexpr int kFW = kFT / 32;   // warps per CTA
-constexpr int kCombineMaxParts = 512;
+constexpr int kStages = 3;                 // ring stages of a rows item (16 rows of K + 16 rows of V each)
+constexpr int kStageBytes = 2 * 16 * kD * 2;
 
 // Monotone map float -> uint32 (larger float => larger key); key 0 is free to mean "not eligible".
 __device__ __forceinline__ uint32_t order_key(float x) {
@@ -38,37 +42,431 @@ __device__ __forceinline__ uint32_t order_key(float x) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-struct ZDesc { int32_t valid, miss, len, rr, way; uint32_t bytes; };
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-struct __align__(16) Shared {
-  uint64_t bars[2];
-  ZDesc desc[2];
-  int32_t item, flag, scan[kFW + 1], misc[4];
-  float ml[kFW * SEKV_MAX_GROUP * 2];
-};
-
-// ---------------------------------------------------------------------------------------------------
-// a7: merge the warps' results of one CTA and store one partial (m2, l, o[128]) per head.
-// ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void cta_merge_store(float* sm_o, float* sm_ml, float* __restrict__ out) {
-  __syncthreads();
-  for (int o = threadIdx.x; o < G * kD; o += kFT) {
-    const int h = o / kD, d = o % kD;
-    float mm = -INFINITY;
+__device__ __forceinline__ void red_add_release(int32_t* p, int v) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ int warp_sum_i(int v) {
 #pragma unroll
-    for (int w = 0; w < kFW; ++w) mm = fmaxf(mm, sm_ml[(w * G + h) * 2]);
-    float ls = 0.f, os = 0.f;
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+// exclusive prefix sum over the warp
+__device__ __forceinline__ int warp_excl_scan(int v, int lane) {
+  int s = v;
 #pragma unroll
-    for (int w = 0; w < kFW; ++w) {
-      const float mw = sm_ml[(w * G + h) * 2];
-      const float c = (mw == -INFINITY) ? 0.f : exp2f(mw - mm);
-      ls = fmaf(sm_ml[(w * G + h) * 2 + 1], c, ls);
-      os = fmaf(sm_o[(w * G + h) * kD + d], c, os);
-    }
-    if (d == 0) { out[h * kPartStride] = mm; out[h * kPartStride + 1] = ls; }
-    out[h * kPartStride + 4 + d] = os;
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, s, o);
+    if (lane >= o) s += t;
   }
+  return s - v;
+}
+
+// per-group counters inside P.ctrs
+__device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
+enum { C_QP = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };
+
+// spin (lane 0) until the counter reaches `target`
+// (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
+__device__ __forceinline__ void wait_ctr(const int32_t* c, int target, int lane, unsigned long long* t_mid = nullptr) {
+  if (lane == 0) {
+    int v;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
+      if (v >= target) break;
+      __nanosleep(64);
+    }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+    if (t_mid) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(*t_mid));
+  }
+  __syncwarp();
+}
+// trace mark k (1..3) of the current item (lane 0; tm = null when tracing is off)
+__device__ __forceinline__ void mark(unsigned long long* tm, int k, int lane) {
+  if (tm && lane == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tm[k]));
+}
+// every lane's earlier global writes happen-before the counter increment: __syncwarp orders them before
+// lane 0's release (cumulativity), so no separate fence is needed
+__device__ __forceinline__ void signal_ctr(int32_t* c, int lane) {
+  __syncwarp();
+  if (lane == 0) red_add_release(c, 1);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a1 (Eq. 4): q'[j] = sum_d W[h][j][d] q[h][d] for one query head.  W_h is dp x 128 bf16, contiguous: load i of
+// the warp covers rows 2i and 2i+1 (512 bytes); lane L holds 8 elements d = 8 (L & 15) .. of row 2i + (L >> 4).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void qproj_item(const FusedParams& P, const Item& I, int lane) {
+  const int b = I.bg / P.Hkv, g = I.bg % P.Hkv;
+  const int G = P.Hq / P.Hkv;
+  const int h = g * G + I.a;
+  const __nv_bfloat16* q = P.q + ((size_t)b * P.Hq + h) * kD + 8 * (lane & 15);
+  const uint4 qv = *reinterpret_cast<const uint4*>(q);
+  const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)h * P.dp * kD * 2 + lane * 16;
+  float qf[8];
+  {
+    const uint32_t w[4] = {qv.x, qv.y, qv.z, qv.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) { qf[2 * e] = __uint_as_float(w[e] << 16); qf[2 * e + 1] = __uint_as_float(w[e] & 0xffff0000u); }
+  }
+  float* dst = P.qp + ((size_t)I.bg * G + I.a) * P.dp;
+#pragma unroll 1
+  for (int i0 = 0; i0 < P.dp / 2; i0 += 4) {
+    uint4 wv[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i0 + u < P.dp / 2) wv[u] = ldg16(Wh + (size_t)(i0 + u) * 512);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (i0 + u < P.dp / 2) {
+        const uint32_t w[4] = {wv[u].x, wv[u].y, wv[u].z, wv[u].w};
+        float acc = 0.f;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          acc = fmaf(__uint_as_float(w[e] << 16), qf[2 * e], acc);
+          acc = fmaf(__uint_as_float(w[e] & 0xffff0000u), qf[2 * e + 1], acc);
+        }
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if ((lane & 15) == 0) dst[2 * (i0 + u) + (lane >> 4)] = acc;
+      }
+    }
+  }
+  signal_ctr(grp_ctr(P, I.bg, C_QP), lane);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a2 + GQA reduce of a3 (Eq. 5, Eq. 9): spans [I.a, I.b) of (b, g).  The G x nsp rows of the routing table
+// (dp bf16 each) are staged into the warp's region by 16-byte cp.async copies -- all in flight at once,
+// issued before the wait on q' -- and scored from shared memory with compact loops (the code footprint
+// matters more than the arithmetic here: every item runs this once).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, uint8_t* region, int lane,
+                                           unsigned long long* tm) {
+  const int bg = I.bg, g = bg % P.Hkv, G = P.Hq / P.Hkv, dp = P.dp, lpr = dp >> 3;
+  const int nsp = I.b - I.a;
+  const uint8_t* route = (const uint8_t*)P.lv.route;
+  const int total = nsp * G * lpr;
+#pragma unroll 2
+  for (int i = lane; i < total; i += 32) {
+    const int c = i % lpr, t = i / lpr;
+    const int hl = t / nsp, s = t - hl * nsp;
+    cp_async16(region + (size_t)i * 16,
+               route + ((size_t)(g * G + hl) * P.route_head_stride + (size_t)(I.span0 + I.a + s) * dp) * 2 + c * 16);
+  }
+  cp_async_commit();
+  float* sqp = reinterpret_cast<float*>(region + (size_t)P.route_spans * G * dp * 2);     // [G][dp]
+  wait_ctr(grp_ctr(P, bg, C_QP), G, lane, tm);
+  for (int i = lane; i < G * dp; i += 32) sqp[i] = __ldcg(P.qp + (size_t)bg * G * dp + i);
+  cp_async_wait<0>();
+  __syncwarp();
+  mark(tm, 1, lane);
+  const float inv_sqrt_dp = rsqrtf((float)dp);
+  uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
+  for (int s = lane; s < nsp; s += 32) {
+    const float lnl = P.cv.ln_len[I.span0 + I.a + s];
+    float X = -INFINITY;
+    bool elig = (P.tau == nullptr);
+#pragma unroll 1
+    for (int hl = 0; hl < G; ++hl) {
+      const uint4* row = reinterpret_cast<const uint4*>(region + ((size_t)hl * nsp + s) * dp * 2);
+      const float4* qv = reinterpret_cast<const float4*>(sqp + hl * dp);
+      float acc = 0.f;
+#pragma unroll 1
+      for (int c = 0; c < lpr; ++c) {
+        const uint4 v = row[c];
+        const float4 q0 = qv[2 * c], q1 = qv[2 * c + 1];
+        acc = fmaf(__uint_as_float(v.x << 16), q0.x, acc); acc = fmaf(__uint_as_float(v.x & 0xffff0000u), q0.y, acc);
+        acc = fmaf(__uint_as_float(v.y << 16), q0.z, acc); acc = fmaf(__uint_as_float(v.y & 0xffff0000u), q0.w, acc);
+        acc = fmaf(__uint_as_float(v.z << 16), q1.x, acc); acc = fmaf(__uint_as_float(v.z & 0xffff0000u), q1.y, acc);
+        acc = fmaf(__uint_as_float(v.w << 16), q1.z, acc); acc = fmaf(__uint_as_float(v.w & 0xffff0000u), q1.w, acc);
+      }
+      const float x = fmaf(acc, inv_sqrt_dp, lnl);            // Eq. 5, pre-sigmoid logit
+      const float a = 1.f / (1.f + __expf(-x));
+      const int h = g * G + hl;
+      if (P.logits_out) P.logits_out[(size_t)h * P.m_tot + I.span0 + I.a + s] = x;
+      if (P.alpha_out) P.alpha_out[(size_t)h * P.m_tot + I.span0 + I.a + s] = a;
+      if (P.tau != nullptr && a > P.tau[h]) elig = true;       // Eq. 9
+      X = fmaxf(X, x);
+    }
+    gkeys[I.a + s] = elig ? order_key(X) : 0u;
+  }
+  mark(tm, 2, lane);
+  signal_ctr(grp_ctr(P, bg, C_ROUTE), lane);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a3: descending bitonic sort of n (power of two) 64-bit keys in the warp's region
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bitonic_sort_desc_warp(unsigned long long* keys, int n, int lane) {
+  for (int size = 2; size <= n; size <<= 1) {
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = lane; i < (n >> 1); i += 32) {
+        const int lo = ((i & ~(stride - 1)) << 1) | (i & (stride - 1));
+        const int hi = lo | stride;
+        const bool desc = ((lo & size) == 0);
+        const unsigned long long a = keys[lo], c = keys[hi];
+        if ((a < c) == desc) { keys[lo] = c; keys[hi] = a; }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a4: residency plan of (b, g) by one warp.  The device factor cache of a (layer, sequence, kv head) is
+// `ways` slots with a tag (span id) and a stamp (step of last use).  The first n_zoom entries of sh_ids
+// are this step's zoom set: resident ones are hits, the others are demand misses and take the
+// least-recently-used slots not needed by this step.  Entries n_zoom .. n_cand-1 are prefetch candidates
+// (the next-best spans by routing score): the non-resident ones get a slot too and are copied by the
+// side-stream prefetch kernel after this layer's kernel.  Also: zoom bit-mask for the coarse items (an
+// expanded span's coarse entry is replaced by its tokens), de-duplication of
+// caller-supplied ids, one descriptor per expanded span for the ZOOM items, statistics.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void plan_warp(const FusedParams& P, const Item& I, uint8_t* region, int lane, int n_zoom,
+                                          int n_cand, bool dedupe, uint32_t epoch) {
+  const int bg = I.bg, g = bg % P.Hkv;
+  const int span0 = I.span0, m = I.b, ways = P.ways;
+  int32_t* sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
+  int16_t* way_of = reinterpret_cast<int16_t*>(region + P.sm_wayof);
+  int32_t* sh_tag = reinterpret_cast<int32_t*>(region + P.sm_tags);
+  uint32_t* sh_stamp = reinterpret_cast<uint32_t*>(sh_tag + ways);
+  int32_t* sh_victim = reinterpret_cast<int32_t*>(sh_stamp + ways);
+  uint32_t* sh_mask = reinterpret_cast<uint32_t*>(region + P.sm_mask);
+  int32_t* tags = P.lv.tags + (size_t)bg * ways;
+  uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
+  uint32_t* items = P.lv.items + (size_t)bg * P.kc;
+  int32_t* item_span = P.lv.item_span + (size_t)bg * P.kc;
+  ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
+  const uint32_t cur = epoch;
+  for (int w = lane; w < P.mask_words; w += 32) sh_mask[w] = 0u;
+  for (int s = lane; s < m; s += 32) way_of[s] = (int16_t)-1;
+  for (int w = lane; w < ways; w += 32) { sh_tag[w] = tags[w]; sh_stamp[w] = stamps[w]; sh_victim[w] = -1; }
+  __syncwarp();
+  for (int w = lane; w < ways; w += 32) { const int t = sh_tag[w]; if (t >= 0 && t < m) way_of[t] = (int16_t)w; }
+  __syncwarp();
+  unsigned long long n_hit = 0, n_miss = 0, bytes_algo = 0, bytes_h2d = 0, n_pf = 0, bytes_pf = 0;
+  // pass 1: validate / de-duplicate, zoom mask, residency lookup
+  for (int j = lane; j < n_cand; j += 32) {
+    int id = sh_ids[j];
+    if (id < 0 || id >= m) id = -1;
+    const bool zoom = j < n_zoom;
+    if (id >= 0 && zoom) {
+      const uint32_t bit = 1u << (id & 31);
+      const uint32_t old = atomicOr(&sh_mask[id >> 5], bit);
+      if (dedupe && (old & bit)) id = -1;                      // duplicate of an id seen before: dropped
+    }
+    int way = -1;
+    if (id >= 0) {
+      way = way_of[id];
+      if (way >= 0) sh_stamp[way] = cur;
+      const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + id];
+      const int rk = rr & 0xff, rv = (rr >> 8) & 0xff;
+      const int len = P.cv.span_len[span0 + id];
+      const unsigned long long bb = blob_dims(2, len, rk, rv).bytes;
+      if (zoom) {
+        bytes_algo += (unsigned long long)(rk + rv) * (len + kD) * 2 + 4ull * (rk + rv);
+        if (way >= 0) ++n_hit; else { ++n_miss; bytes_h2d += bb; }
+      } else if (way < 0) { ++n_pf; bytes_pf += bb; }
+    }
+    sh_ids[j] = id;
+    item_span[j] = id;
+    items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
+  }
+  __syncwarp();
+  // victims: the n_need oldest ways not used by this step (ties to the lower way), found by repeated
+  // extraction of the minimum (stamp, way) -- only as many as this step has misses
+  const int n_need = min(warp_sum_i((int)(n_miss + n_pf)), ways);
+  for (int v = 0; v < n_need; ++v) {
+    unsigned long long best = ~0ull;
+    for (int w = lane; w < ways; w += 32)
+      if (sh_stamp[w] != cur) best = min(best, ((unsigned long long)sh_stamp[w] << 32) | (unsigned long long)w);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, o));
+    if (best == ~0ull) break;
+    const int w = (int)(best & 0xffffffffull);
+    if (lane == 0) { sh_victim[v] = w; sh_stamp[w] = cur; }    // marked used: not extracted again
+    __syncwarp();
+  }
+  // pass 2: misses take victims in item order; descriptors of the zoom set
+  int miss_base = 0;
+  for (int j0 = 0; j0 < n_cand; j0 += 32) {
+    const int j = j0 + lane;
+    const int id = (j < n_cand) ? sh_ids[j] : -1;
+    uint32_t it = (j < n_cand) ? items[j] : 0u;
+    const bool miss = id >= 0 && it == 0xFFFFFFFFu;
+    const unsigned bal = __ballot_sync(0xffffffffu, miss);
+    if (miss) {
+      const int vi = miss_base + __popc(bal & ((1u << lane) - 1u));
+      const int way = vi < ways ? sh_victim[vi] : -1;
+      if (way >= 0) {
+        sh_tag[way] = id;
+        sh_stamp[way] = cur;
+        it = (uint32_t)way | 0x80000000u;
+      } else {
+        it = 0xC0000000u;                                      // no free slot: fetch, do not keep
+      }
+      items[j] = it;
+    }
+    miss_base += __popc(bal);
+    if (j < n_zoom) {
+      ZDescG d;
+      d.src = 0ull; d.bytes = 0u; d.len = 0; d.rr = 0; d.way_miss = it; d.id = id; d.pad = 0;
+      if (id >= 0) {
+        const int gs = span0 + id;
+        d.rr = P.lv.dir_rank[(size_t)g * P.spans_cap + gs];
+        d.len = P.cv.span_len[gs];
+        d.bytes = (uint32_t)blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff).bytes;
+        const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
+                                                : P.lv.slots + ((size_t)bg * ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
+        d.src = (unsigned long long)src;
+      }
+      zd[j] = d;
+    }
+  }
+  __syncwarp();
+  for (int w = lane; w < ways; w += 32) { tags[w] = sh_tag[w]; stamps[w] = sh_stamp[w]; }
+  uint32_t* gmask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
+  for (int w = lane; w < P.mask_words; w += 32) gmask[w] = sh_mask[w];
+  if (lane == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    n_hit += __shfl_xor_sync(0xffffffffu, n_hit, o);
+    n_miss += __shfl_xor_sync(0xffffffffu, n_miss, o);
+    bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
+    bytes_h2d += __shfl_xor_sync(0xffffffffu, bytes_h2d, o);
+    n_pf += __shfl_xor_sync(0xffffffffu, n_pf, o);
+    bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
+  }
+  if (lane == 0) {
+    if (n_hit) atomicAdd(&P.stats[ST_HITS], n_hit);
+    if (n_miss) atomicAdd(&P.stats[ST_MISSES], n_miss);
+    if (n_hit + n_miss) { atomicAdd(&P.stats[ST_ZOOMED], n_hit + n_miss); atomicAdd(&P.stats[ST_SKIPPED], n_hit + n_miss); }
+    if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
+    if (bytes_h2d + bytes_pf) atomicAdd(&P.stats[ST_H2D], bytes_h2d + bytes_pf);
+    if (n_pf) atomicAdd(&P.stats[ST_PREFETCHED], n_pf);
+  }
+  signal_ctr(grp_ctr(P, bg, C_PLAN), lane);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a3 (Eq. 9, cap L123): top-n_cand of the group's m keys by one warp.  4-pass radix select (8 bits per
+// pass, shared-memory histogram) finds the n_cand-th largest key T; keys > T are taken, keys == T are
+// taken in increasing span id until the count is met (ties to the lower id); the <= kc winners are
+// then sorted by (key descending, id ascending).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void select_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch, unsigned long long* tm) {
+  const int bg = I.bg, m = I.b;
+  int32_t* sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
+  if (!(P.mode & FM_ROUTE)) {
+    // caller-supplied zoom set (sekv_decode_attn)
+    int cnt = 0;
+    if (P.ids != nullptr && P.count != nullptr) cnt = max(0, min(P.count[bg], P.k_cap));
+    const int32_t* src = P.ids + (size_t)bg * max(P.k_cap, 1);
+    for (int j = lane; j < cnt; j += 32) sh_ids[j] = src[j];
+    __syncwarp();
+    plan_warp(P, I, region, lane, cnt, cnt, true, epoch);
+    return;
+  }
+  uint32_t* keys = reinterpret_cast<uint32_t*>(region);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(region + P.sm_hist);
+  unsigned long long* cand = reinterpret_cast<unsigned long long*>(region + P.sm_cand);
+  wait_ctr(grp_ctr(P, bg, C_ROUTE), I.a, lane, tm);
+  const uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
+  int ne = 0;
+  for (int i = lane; i < m; i += 32) {
+    const uint32_t k = __ldcg(gkeys + i);
+    keys[i] = k;
+    ne += (k != 0u);
+  }
+  const int n_elig = warp_sum_i(ne);
+  mark(tm, 1, lane);
+  int cnt = P.k < 0 ? n_elig : min(P.k, n_elig);
+  cnt = min(cnt, P.k_cap);
+  int n_cand = cnt;
+  if (P.k >= 0 && (P.mode & FM_ATTN)) n_cand = min(min(cnt + P.prefetch, n_elig), P.kc);
+  __syncwarp();
+  uint32_t T = 0u;            // threshold key
+  int need = 0;               // keys == T to take
+  if (n_cand == 0) {
+    T = 0xFFFFFFFFu;
+  } else if (n_cand < n_elig) {
+    uint32_t prefix = 0u, maskb = 0u;
+    need = n_cand;
+    for (int shift = 24; shift >= 0; shift -= 8) {
+      for (int i = lane; i < 256; i += 32) hist[i] = 0u;
+      __syncwarp();
+#pragma unroll 4
+      for (int i = lane; i < m; i += 32) {
+        const uint32_t k = keys[i];
+        if (k != 0u && (k & maskb) == prefix) atomicAdd(&hist[(k >> shift) & 255u], 1u);
+      }
+      __syncwarp();
+      int loc[8], tot = 0;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { loc[e] = (int)hist[255 - (8 * lane + e)]; tot += loc[e]; }
+      int run = warp_excl_scan(tot, lane);       // matching keys in bins above this lane's bins
+      int found = -1, fb = 0;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        if (found < 0 && run < need && run + loc[e] >= need) { found = 255 - (8 * lane + e); fb = run; }
+        run += loc[e];
+      }
+      const unsigned bal = __ballot_sync(0xffffffffu, found >= 0);
+      const int srcl = __ffs(bal) - 1;
+      const int d = __shfl_sync(0xffffffffu, found, srcl);
+      fb = __shfl_sync(0xffffffffu, fb, srcl);
+      need -= fb;
+      prefix |= (uint32_t)d << shift;
+      maskb |= 255u << shift;
+      __syncwarp();
+    }
+    T = prefix;
+  }
+  mark(tm, 2, lane);
+  // ordered compaction: lane owns a contiguous block of span ids
+  const int per = (m + 31) / 32;
+  const int lo = min(m, lane * per), hi = min(m, lo + per);
+  int gt = 0, eq = 0;
+  for (int i = lo; i < hi; ++i) { const uint32_t k = keys[i]; gt += (k > T); eq += (k == T); }
+  const int eq_before = warp_excl_scan(eq, lane);
+  const int take_eq = (T == 0u) ? 0 : max(0, min(eq, need - eq_before));
+  int pos = warp_excl_scan(gt + take_eq, lane);
+  int taken = 0;
+  for (int i = lo; i < hi; ++i) {
+    const uint32_t k = keys[i];
+    bool sel = k > T;
+    if (k == T && taken < take_eq) { sel = true; ++taken; }
+    if (sel && pos < P.kc) cand[pos++] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
+  }
+  __syncwarp();
+  if (n_cand <= 64) {
+    for (int j = lane; j < n_cand; j += 32) {
+      const unsigned long long mine = cand[j];
+      int r = 0;
+      for (int i = 0; i < n_cand; ++i) r += (cand[i] > mine);
+      sh_ids[r] = (int32_t)(0xFFFFFFFFu - (uint32_t)(mine & 0xFFFFFFFFull));
+    }
+  } else {
+    int n2 = 64;
+    while (n2 < n_cand) n2 <<= 1;
+    for (int j = n_cand + lane; j < n2; j += 32) cand[j] = 0ull;
+    __syncwarp();
+    bitonic_sort_desc_warp(cand, n2, lane);
+    for (int j = lane; j < n_cand; j += 32) sh_ids[j] = (int32_t)(0xFFFFFFFFu - (uint32_t)(cand[j] & 0xFFFFFFFFull));
+  }
+  __syncwarp();
+  int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
+  for (int j = lane; j < P.k_cap; j += 32) my_ids[j] = j < cnt ? sh_ids[j] : -1;
+  if (lane == 0) P.count[bg] = cnt;
+  mark(tm, 3, lane);
+  if (P.mode & FM_ATTN) plan_warp(P, I, region, lane, cnt, n_cand, false, epoch);
 }
 
 __device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q, int G, int gid, int t4,
@@ -81,30 +479,68 @@ __device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q
   }
 }
 
+// one partial record (m2, l, pad, pad, o[128]) per head; lane (gid, t4) holds head gid's (m, l) and the
+// accumulators listed by the callers
+__device__ __forceinline__ float* part_ptr(const FusedParams& P, const Item& I, int hl) {
+  return P.partials + ((size_t)I.pbase + (size_t)hl * I.np + I.part) * kPartStride;
+}
+
 // ---------------------------------------------------------------------------------------------------
-// a5: rows [row_begin, row_end) of the entry table of (b, g): pool tokens (logit = q.K/sqrt(d)) and
-// unexpanded coarse entries (logit = q.k_bar/sqrt(d) + ln|S|, value v_bar).
-//   QK^T : lane (gid = lane/4, t4 = lane%4) loads 16-byte chunk (t4 + 4j) of the K row of token gid; its
-//          four words are the (b0,b1) pairs of two k-steps; Q is loaded the same way (the contraction
-//          index may be permuted consistently on both operands).
+// a5: rows [I.a, I.b) of the entry table of (b, g): pool tokens (logit = q.K/sqrt(d)) and unexpanded coarse
+// entries (logit = q.k_bar/sqrt(d) + ln|S|, value v_bar).  16-row tiles of K and V
+// stream through a kStages-deep cp.async ring in the warp's region.  Shared-memory layout of a stage:
+// K rows then V rows, 256 bytes per row, 16-byte chunk c of row r stored at chunk c ^ ((r & 1) << 2)
+// (K) or c ^ (((r >> 1) & 3) << 1) (V): both fragment access patterns below are bank-conflict free.
+//   QK^T : lane (gid = lane/4, t4 = lane%4) reads chunk (t4 + 4j) of the K row of token gid; its four
+//          words are the (b0,b1) pairs of two k-steps; Q is loaded the same way (the contraction index
+//          may be permuted consistently on both operands).
 //   P V  : computed transposed, O^T = V^T P^T (M = 16 dims, N = 8 heads, K = 16 tokens): the C fragment
 //          of S IS the B fragment of P^T.  P (fp32) is split into bf16 hi + lo parts and multiplied
 //          twice, so probabilities carry ~16 bits.
 // ---------------------------------------------------------------------------------------------------
 template <int G>
-__device__ __forceinline__ void rows_item(const FusedParams& P, int bg, int row_begin, int row_end, float* sm_o,
-                                          float* sm_ml, float* __restrict__ partial_out) {
-  const int b = bg / P.Hkv, g = bg % P.Hkv;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, unsigned long long* tm) {
+  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
-  const int A = P.cv.seq_pool_cnt[b];
-  const int row0 = P.cv.seq_row_off[b];
-  const int span0 = P.cv.seq_span_off[b];
-  const uint8_t* Kb = (const uint8_t*)P.lv.ent_k + ((size_t)g * P.ent_head_stride + (size_t)row0 * kD) * 2;
-  const uint8_t* Vb = (const uint8_t*)P.lv.ent_v + ((size_t)g * P.ent_head_stride + (size_t)row0 * kD) * 2;
-  const uint32_t* mask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
+  const int A = I.A, row_begin = I.a, row_end = I.b;
+  const uint8_t* Kb = (const uint8_t*)P.lv.ent_k + ((size_t)g * P.ent_head_stride + (size_t)I.row0 * kD) * 2;
+  const uint8_t* Vb = (const uint8_t*)P.lv.ent_v + ((size_t)g * P.ent_head_stride + (size_t)I.row0 * kD) * 2;
   const float scale2 = rsqrtf((float)kD) * kLog2e;
+  const int ntiles = (row_end - row_begin + 15) >> 4;
 
+  auto fill = [&](int t) {
+    uint8_t* Ks = region + (t % kStages) * kStageBytes;
+    uint8_t* Vs = Ks + 16 * kD * 2;
+    const int r0 = row_begin + t * 16;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int idx = lane + 32 * i, r = idx >> 4, c = idx & 15;
+      const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + c * 16;
+      cp_async16(Ks + r * 256 + ((c ^ ((r & 1) << 2)) << 4), Kb + src);
+      cp_async16(Vs + r * 256 + ((c ^ (((r >> 1) & 3) << 1)) << 4), Vb + src);
+    }
+  };
+#pragma unroll
+  for (int t = 0; t < kStages; ++t) {
+    if (t < ntiles) fill(t);
+    cp_async_commit();
+  }
+  // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L
+  float bias_reg[2] = {0.f, 0.f};
+  if (I.kind == IT_COARSE) {
+    wait_ctr(grp_ctr(P, bg, C_PLAN), 1, lane, tm);
+    const uint32_t* mask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int row = row_begin + 32 * u + lane;
+      float bv = -INFINITY;
+      if (row < row_end) {
+        const int s = row - A;
+        bv = (__ldcg(mask + (s >> 5)) & (1u << (s & 31))) ? -INFINITY : P.cv.ln_len[I.span0 + s] * kLog2e;
+      }
+      bias_reg[u] = bv;
+    }
+  }
   uint32_t qf[4][4];
   load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
   float m_run = -INFINITY, l_run = 0.f;
@@ -115,47 +551,28 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, int bg, int row_
 #pragma unroll
     for (int w = 0; w < 4; ++w) { acc[s][w][0] = 0.f; acc[s][w][1] = 0.f; acc[s][w][2] = 0.f; acc[s][w][3] = 0.f; }
 
-  const int ntiles = (row_end - row_begin + 15) >> 4;
-  uint4 kf[2][4], vf[4][2];
-  auto load_k = [&](int t) {
-    const int r0 = row_begin + t * 16;
-#pragma unroll
-    for (int nt = 0; nt < 2; ++nt) {
-      const int row = min(r0 + 8 * nt + gid, row_end - 1);
-      const uint8_t* p = Kb + (size_t)row * (kD * 2) + t4 * 16;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) kf[nt][j] = ldg16(p + j * 64);
-    }
-  };
-  auto load_v = [&](int t) {
-    const int r0 = row_begin + t * 16;
-#pragma unroll
-    for (int rr = 0; rr < 4; ++rr) {
-      const int row = min(r0 + 2 * t4 + (rr & 1) + 8 * (rr >> 1), row_end - 1);
-      const uint8_t* p = Vb + (size_t)row * (kD * 2) + gid * 16;
-      vf[rr][0] = ldg16(p);
-      vf[rr][1] = ldg16(p + 128);
-    }
-  };
-  if (warp < ntiles) { load_k(warp); load_v(warp); }
-  for (int t = warp; t < ntiles; t += kFW) {
+  for (int t = 0; t < ntiles; ++t) {
+    cp_async_wait<kStages - 1>();
+    __syncwarp();
+    const uint8_t* Ks = region + (t % kStages) * kStageBytes;
+    const uint8_t* Vs = Ks + 16 * kD * 2;
     const int r0 = row_begin + t * 16;
     float sacc[2][4];
 #pragma unroll
     for (int nt = 0; nt < 2; ++nt) {
       sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
+      const int r = 8 * nt + gid;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        mma16816(sacc[nt], qf[j][0], qf[j][1], kf[nt][j].x, kf[nt][j].y);
-        mma16816(sacc[nt], qf[j][2], qf[j][3], kf[nt][j].z, kf[nt][j].w);
+        const uint4 kv = *reinterpret_cast<const uint4*>(Ks + r * 256 + (((t4 + 4 * j) ^ ((r & 1) << 2)) << 4));
+        mma16816(sacc[nt], qf[j][0], qf[j][1], kv.x, kv.y);
+        mma16816(sacc[nt], qf[j][2], qf[j][3], kv.z, kv.w);
       }
     }
-    const bool more = (t + kFW) < ntiles;
-    if (more) load_k(t + kFW);
     // logits in the base-2 domain with the entry bias (0 for pool tokens, ln|S| for coarse entries,
     // -inf for expanded spans and for rows past the item)
     float z[2][2];
-    if (r0 + 16 <= min(A, row_end)) {     // warp-uniform fast path: all pool tokens
+    if (I.kind == IT_POOL && r0 + 16 <= row_end) {     // warp-uniform fast path
 #pragma unroll
       for (int nt = 0; nt < 2; ++nt) { z[nt][0] = sacc[nt][0] * scale2; z[nt][1] = sacc[nt][1] * scale2; }
     } else {
@@ -163,13 +580,14 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, int bg, int row_
       for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          const int row = r0 + 8 * nt + 2 * t4 + e;
+          const int ri = 16 * t + 8 * nt + 2 * t4 + e;      // row index within the item
           float bias = 0.f;
-          if (row >= row_end) bias = -INFINITY;
-          else if (row >= A) {
-            const int s = row - A;
-            bias = (__ldcg(mask + (s >> 5)) & (1u << (s & 31))) ? -INFINITY : P.cv.ln_len[span0 + s] * kLog2e;
+          if (I.kind == IT_COARSE) {
+            const float b0 = __shfl_sync(0xffffffffu, bias_reg[0], ri & 31);
+            const float b1 = __shfl_sync(0xffffffffu, bias_reg[1], ri & 31);
+            bias = (ri < 32) ? b0 : b1;
           }
+          if (row_begin + ri >= row_end) bias = -INFINITY;
           z[nt][e] = fmaf(sacc[nt][e], scale2, bias);
         }
     }
@@ -195,10 +613,16 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, int bg, int row_
     split_bf16(p10, p11, b1h, b1l);
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-      const uint32_t ra[4] = {vf[0][s].x, vf[0][s].y, vf[0][s].z, vf[0][s].w};
-      const uint32_t rb[4] = {vf[1][s].x, vf[1][s].y, vf[1][s].z, vf[1][s].w};
-      const uint32_t rc[4] = {vf[2][s].x, vf[2][s].y, vf[2][s].z, vf[2][s].w};
-      const uint32_t rd[4] = {vf[3][s].x, vf[3][s].y, vf[3][s].z, vf[3][s].w};
+      uint4 vf[4];
+#pragma unroll
+      for (int rr = 0; rr < 4; ++rr) {
+        const int r = 2 * t4 + (rr & 1) + 8 * (rr >> 1);
+        vf[rr] = *reinterpret_cast<const uint4*>(Vs + r * 256 + (((gid + 8 * s) ^ (t4 << 1)) << 4));
+      }
+      const uint32_t ra[4] = {vf[0].x, vf[0].y, vf[0].z, vf[0].w};
+      const uint32_t rb[4] = {vf[1].x, vf[1].y, vf[1].z, vf[1].w};
+      const uint32_t rc[4] = {vf[2].x, vf[2].y, vf[2].z, vf[2].w};
+      const uint32_t rd[4] = {vf[3].x, vf[3].y, vf[3].z, vf[3].w};
 #pragma unroll
       for (int w = 0; w < 4; ++w) {
         const uint32_t a0 = __byte_perm(ra[w], rb[w], 0x5410), a1 = __byte_perm(ra[w], rb[w], 0x7632);
@@ -207,35 +631,40 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, int bg, int row_
         mma16816_full(acc[s][w], a0, a1, a2, a3, b0l, b1l);
       }
     }
-    if (more) load_v(t + kFW);
+    __syncwarp();                                      // every lane is done with this stage
+    if (t + kStages < ntiles) fill(t + kStages);
+    cp_async_commit();
   }
+  cp_async_wait<0>();
   l_run = quad_sum(l_run);
-  if (gid < G && t4 == 0) { sm_ml[(warp * G + gid) * 2] = m_run; sm_ml[(warp * G + gid) * 2 + 1] = l_run; }
+  if (gid < G && t4 == 0) {
+    float* pp = part_ptr(P, I, gid);
+    pp[0] = m_run; pp[1] = l_run;
+  }
 #pragma unroll
   for (int c = 0; c < 2; ++c) {
     const int hh = 2 * t4 + c;
     if (hh < G) {
-      float* o = sm_o + (warp * G + hh) * kD;
+      float* o = part_ptr(P, I, hh) + 4;
 #pragma unroll
       for (int s = 0; s < 2; ++s)
 #pragma unroll
-        for (int w = 0; w < 4; ++w) {
-          o[64 * s + 8 * gid + 2 * w] = acc[s][w][c];
-          o[64 * s + 8 * gid + 2 * w + 1] = acc[s][w][2 + c];
-        }
+        for (int w = 0; w < 4; ++w)
+          *reinterpret_cast<float2*>(o + 64 * s + 8 * gid + 2 * w) = make_float2(acc[s][w][c], acc[s][w][2 + c]);
     }
   }
-  cta_merge_store<G>(sm_o, sm_ml, partial_out);
+  signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a6: one expanded span, blob resident in shared memory; the CTA's warps split its 16-token chunks.
+// a6: one expanded span, blob resident in the warp's region; the warp walks its 16-token chunks.
 //   c = sigma_K o (Vt_K q) * log2e/sqrt(d)   (rows of Vt_K play the role of tokens in QK^T)
 //   logits = U_K c  (= (U Sigma V^T q), Eq. 8 never materialised), p = 2^(z - m)
 //   y = p^T U_V,   o += (sigma_V o y) V_V^T  accumulated into the warp's running (M, L, of)
 // ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDims& bd, int warp, int lane,
+// NK: compile-time bound on the 16-wide k-steps over the key and value ranks (1, 2 or 4)
+template <int G, int NK>
+__device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDims& bd, int lane,
                                                const uint32_t (&qf)[4][4], float& M, float& L, float (&of)[16][4]) {
   const int gid = lane >> 2, t4 = lane & 3;
   const float* sK = (const float*)(blob + bd.off_sk);
@@ -244,12 +673,11 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   const uint8_t* VV = blob + bd.off_vv;
   const int nks = (bd.rkp + 15) >> 4, nvs = (bd.rvp + 15) >> 4;     // k-steps over the key / value rank
   const int ngrp = bd.lenp >> 4;
-  if (warp >= ngrp) return;                                          // warp-uniform: nothing for this warp
   const float scale2 = rsqrtf((float)kD) * kLog2e;
   // 1. c
-  uint32_t ckh[4][2], ckl[4][2];
+  uint32_t ckh[NK][2], ckl[NK][2];
 #pragma unroll
-  for (int ks = 0; ks < 4; ++ks) {
+  for (int ks = 0; ks < NK; ++ks) {
     ckh[ks][0] = ckh[ks][1] = ckl[ks][0] = ckl[ks][1] = 0u;
     if (ks < nks) {
 #pragma unroll
@@ -276,10 +704,10 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   }
   // 2. the warp's token chunks
   float m_s = -INFINITY, l_s = 0.f;
-  float yf[8][4];
+  float yf[2 * NK][4];
 #pragma unroll
-  for (int n = 0; n < 8; ++n) { yf[n][0] = yf[n][1] = yf[n][2] = yf[n][3] = 0.f; }
-  for (int grp = warp; grp < ngrp; grp += kFW) {
+  for (int n = 0; n < 2 * NK; ++n) { yf[n][0] = yf[n][1] = yf[n][2] = yf[n][3] = 0.f; }
+  for (int grp = 0; grp < ngrp; ++grp) {
     const uint8_t* UKc = blob + bd.off_chunks + (size_t)grp * bd.chunk_bytes;
     const uint8_t* UVtc = UKc + bd.uvt_in_chunk;
     float sacc[2][4];
@@ -288,7 +716,7 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
       sacc[u][0] = sacc[u][1] = sacc[u][2] = sacc[u][3] = 0.f;
       const uint8_t* prow = UKc + (size_t)pi_index(u, gid) * (bd.rkp * 2) + t4 * 8;
 #pragma unroll
-      for (int ks = 0; ks < 4; ++ks) {
+      for (int ks = 0; ks < NK; ++ks) {
         if (ks < nks) {
           uint2 bv = make_uint2(0u, 0u);
           if (16 * ks + 4 * t4 < bd.rkp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
@@ -310,7 +738,7 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
       const float corr = exp2f(m_s - m_safe);
       l_s *= corr;
 #pragma unroll
-      for (int n = 0; n < 8; ++n) { yf[n][0] *= corr; yf[n][1] *= corr; }
+      for (int n = 0; n < 2 * NK; ++n) { yf[n][0] *= corr; yf[n][1] *= corr; }
     }
     m_s = m_new;
     const float p00 = exp2f(z[0][0] - m_safe), p01 = exp2f(z[0][1] - m_safe);
@@ -321,7 +749,7 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
     split_bf16(p10, p11, a2h, a2l);     // tokens 4*t4 + {2,3}  <-> k = 8 + 2*t4 + e
     // y += P U_V : B[k = token][n = i] read from the transposed factor UVt[i][token]
 #pragma unroll
-    for (int n = 0; n < 8; ++n) {
+    for (int n = 0; n < 2 * NK; ++n) {
       if (n < 2 * nvs) {
         const int irow = pi_index(n, gid);
         uint2 bv = make_uint2(0u, 0u);
@@ -339,9 +767,9 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   M = M_new;
 #pragma unroll
   for (int nd = 0; nd < 16; ++nd) { of[nd][0] *= c_old; of[nd][1] *= c_old; }
-  uint32_t yh[4][2], yl[4][2];          // yf[n][e] is head gid, rank index 16(n>>1) + 4*t4 + 2(n&1) + e
+  uint32_t yh[NK][2], yl[NK][2];          // yf[n][e] is head gid, rank index 16(n>>1) + 4*t4 + 2(n&1) + e
 #pragma unroll
-  for (int ks = 0; ks < 4; ++ks) {
+  for (int ks = 0; ks < NK; ++ks) {
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       yh[ks][u] = yl[ks][u] = 0u;
@@ -357,7 +785,7 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   for (int nd = 0; nd < 16; ++nd) {
     const uint8_t* prow = VV + (size_t)(8 * nd + gid) * (bd.rvp * 2) + t4 * 8;
 #pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
+    for (int ks = 0; ks < NK; ++ks) {
       if (ks < nvs) {
         uint2 bv = make_uint2(0u, 0u);
         if (16 * ks + 4 * t4 < bd.rvp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
@@ -368,488 +796,254 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   }
 }
 
-// wait until the plan of (b, g) has been published for this launch
-__device__ __forceinline__ void wait_plan(const FusedParams& P, int bg, uint32_t epoch) {
-  if (threadIdx.x == 0) {
-    const uint32_t* f = (const uint32_t*)(P.ctrs + 2 + 3 * bg + 2);
-    while (ld_acquire(f) != epoch) __nanosleep(64);
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// lane 0 starts a 1-D bulk copy into the warp's region; every lane waits for its bytes
+__device__ __forceinline__ void region_fetch(uint8_t* region, const void* src, uint32_t bytes, uint64_t* bar,
+                                             uint32_t& phase, int lane) {
+  __syncwarp();                                    // every lane is done with the region's previous contents
+  if (lane == 0) {
+    fence_proxy_async_all();
+    mbar_arrive_expect_tx(bar, bytes);
+    bulk_g2s(region, src, bytes, bar);
   }
-  __syncthreads();
+  mbar_wait(bar, phase);
+  phase ^= 1u;
 }
 
+__device__ __forceinline__ ZDescG load_zdesc(const ZDescG* p) {
+  const uint4 a = __ldcg(reinterpret_cast<const uint4*>(p)), c = __ldcg(reinterpret_cast<const uint4*>(p) + 1);
+  ZDescG d;
+  d.src = (unsigned long long)a.x | ((unsigned long long)a.y << 32);
+  d.bytes = a.z; d.len = (int32_t)a.w; d.rr = (int32_t)c.x; d.way_miss = c.y; d.id = (int32_t)c.z; d.pad = 0;
+  return d;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a4 + a6: plan items [I.a, I.b) of (b, g), one expanded span after the other through the warp's region
+// ---------------------------------------------------------------------------------------------------
 template <int G>
-__device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* dsm, Shared& S, float* sm_o,
-                                          uint32_t (&phase)[2], float* __restrict__ partial_out) {
+__device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
+                                          uint32_t& phase, int lane, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int gid = lane >> 2, t4 = lane & 3;
-  const int n_zoom = __ldcg(P.plan_counts + 2 * bg);
-  const int j0 = I.a, j1 = min(I.b, n_zoom);
-  const int span0 = P.cv.seq_span_off[b];
   uint32_t qf[4][4];
   load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
+  wait_ctr(grp_ctr(P, bg, C_PLAN), 1, lane, tm);
+  const int n_zoom = __ldcg(P.plan_counts + 2 * bg);
+  const int j0 = I.a, j1 = min(I.b, n_zoom);
   float M = -INFINITY, L = 0.f;
   float of[16][4];
 #pragma unroll
   for (int n = 0; n < 16; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
-
-  auto issue = [&](int j) {            // thread 0 only
-    const int buf = (j - j0) & 1;
-    const int id = __ldcg(P.lv.item_span + (size_t)bg * P.kc + j);
-    ZDesc d;
-    d.valid = 0; d.miss = 0; d.len = 0; d.rr = 0; d.way = 0; d.bytes = 0;
-    if (id >= 0) {
-      const uint32_t it = __ldcg(P.lv.items + (size_t)bg * P.kc + j);
-      const int gs = span0 + id;
-      d.valid = 1;
-      d.miss = (it >> 31) & 1;
-      d.way = (int)(it & 0x7FFFFFFFu);
-      d.rr = P.lv.dir_rank[(size_t)g * P.spans_cap + gs];
-      d.len = P.cv.span_len[gs];
-      const BlobDims bd = blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff);
-      d.bytes = (uint32_t)bd.bytes;
-      const uint8_t* src = d.miss ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
-                                  : P.lv.slots + ((size_t)bg * P.ways + d.way) * P.slot_bytes;
-      fence_proxy_async();
-      mbar_arrive_expect_tx(&S.bars[buf], d.bytes);
-      bulk_g2s(dsm + (size_t)buf * P.smem_buf_stride, src, d.bytes, &S.bars[buf]);
-    } else {
-      mbar_arrive(&S.bars[buf]);
-    }
-    S.desc[buf] = d;
-  };
-  if (tid == 0) {
-    if (j0 < j1) issue(j0);
-    if (j0 + 1 < j1) issue(j0 + 1);
-  }
-  __syncthreads();                                 // descriptors visible
+  const ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
+  ZDescG dn;
+  dn.id = -1;
+  if (j0 < j1) dn = load_zdesc(zd + j0);
   for (int j = j0; j < j1; ++j) {
-    const int buf = (j - j0) & 1;
-    mbar_wait(&S.bars[buf], phase[buf]);
-    phase[buf] ^= 1u;
-    const ZDesc d = S.desc[buf];
-    const uint8_t* blob = dsm + (size_t)buf * P.smem_buf_stride;
-    if (d.valid) {
-      const BlobDims bd = blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff);
-      zoom_span_warp<G>(blob, bd, warp, lane, qf, M, L, of);
-      if (d.miss) {                                // demand miss: the blob came over PCIe; keep it in its slot
-        int4* dst = reinterpret_cast<int4*>(P.lv.slots + ((size_t)bg * P.ways + d.way) * P.slot_bytes);
-        const int4* src = reinterpret_cast<const int4*>(blob);
-        for (int i = tid; i < (int)(d.bytes >> 4); i += kFT) dst[i] = src[i];
-      }
+    const ZDescG d = dn;
+    if (j + 1 < j1) dn = load_zdesc(zd + j + 1);
+    if (d.id < 0) continue;
+    region_fetch(region, (const void*)d.src, d.bytes, bar, phase, lane);
+    if (j == j0) mark(tm, 1, lane);
+    const BlobDims bd = blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff);
+    const int kst = (max(bd.rkp, bd.rvp) + 15) >> 4;
+    if (kst <= 1) zoom_span_warp<G, 1>(region, bd, lane, qf, M, L, of);
+    else if (kst == 2) zoom_span_warp<G, 2>(region, bd, lane, qf, M, L, of);
+    else zoom_span_warp<G, 4>(region, bd, lane, qf, M, L, of);
+    if (j == j0) mark(tm, 2, lane);
+    if ((d.way_miss & 0xC0000000u) == 0x80000000u) {   // demand miss: the blob came over PCIe; keep it in its slot
+      int4* dst = reinterpret_cast<int4*>(P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFFFFFu)) * P.slot_bytes);
+      const int4* src = reinterpret_cast<const int4*>(region);
+      for (int i = lane; i < (int)(d.bytes >> 4); i += 32) dst[i] = src[i];
     }
-    __syncthreads();                               // everyone is done with buf (and has read its descriptor)
-    if (tid == 0 && j + 2 < j1) issue(j + 2);
-    if (j + 2 < j1) __syncthreads();               // next descriptor visible (block-uniform condition)
   }
-  // warp results -> shared memory -> one partial
+  mark(tm, 3, lane);
   L = quad_sum(L);
-  float* sm_ml = S.ml;
-  if (gid < G) {
-    if (t4 == 0) { sm_ml[(warp * G + gid) * 2] = M; sm_ml[(warp * G + gid) * 2 + 1] = L; }
-    float* o = sm_o + (warp * G + gid) * kD;          // of[nd][c] is head gid, dimension 8*nd + 2*t4 + c
+  if (gid < G) {                                       // of[nd][c] is head gid, dimension 8*nd + 2*t4 + c
+    float* pp = part_ptr(P, I, gid);
+    if (t4 == 0) { pp[0] = M; pp[1] = L; }
 #pragma unroll
-    for (int nd = 0; nd < 16; ++nd) { o[8 * nd + 2 * t4] = of[nd][0]; o[8 * nd + 2 * t4 + 1] = of[nd][1]; }
+    for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2*>(pp + 4 + 8 * nd + 2 * t4) = make_float2(of[nd][0], of[nd][1]);
   }
-  cta_merge_store<G>(sm_o, sm_ml, partial_out);
+  signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a7: log-sum-exp merge of all partials of (b, g) -> out, lse.  Run by the last attention item of the
-// group to finish.  Warp w takes partials p = w, w+4, ...; lane owns 4 output dimensions.
+// a7 (L61): log-sum-exp merge of the np partials of one query head -> out, lse.  The head's records are
+// contiguous; they move into the warp's region by bulk copies and are reduced from shared memory.
 // ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void combine_group(const FusedParams& P, int bg, uint8_t* dsm, float* sm_o) {
-  const int b = bg / P.Hkv, g = bg % P.Hkv;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int p0 = P.bg_part_base[bg], n = P.bg_part_base[bg + 1] - p0;
-  const float* parts = P.partials + (size_t)p0 * G * kPartStride;
-  float* sh_w = reinterpret_cast<float*>(dsm);                 // [G][kCombineMaxParts] weights, then [G] L, [G] M
-  float* sh_L = sh_w + G * kCombineMaxParts;
-  float* sh_M = sh_L + SEKV_MAX_GROUP;
-  __syncthreads();
-  for (int hl = warp; hl < G; hl += kFW) {
-    float mm = -INFINITY;
-    for (int p = lane; p < n; p += 32) mm = fmaxf(mm, __ldcg(parts + ((size_t)p * G + hl) * kPartStride));
-    mm = warp_max(mm);
-    float ls = 0.f;
+__device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
+                                             uint32_t& phase, int lane, unsigned long long* tm) {
+  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, hl = I.a, np = I.np;
+  const int G = P.Hq / P.Hkv;
+  wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);
+  const float* src = P.partials + ((size_t)I.pbase + (size_t)hl * np) * kPartStride;
+  const int cap = P.region_bytes / (kPartStride * 4);
+  const float* rec = reinterpret_cast<const float*>(region);
+  float M = -INFINITY, L = 0.f;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int p0 = 0; p0 < np; p0 += cap) {
+    const int n = min(cap, np - p0);
+    region_fetch(region, src + (size_t)p0 * kPartStride, (uint32_t)(n * kPartStride * 4), bar, phase, lane);
+    float mc = -INFINITY;
+    for (int p = lane; p < n; p += 32) mc = fmaxf(mc, rec[p * kPartStride]);
+    mc = warp_max(mc);
+    const float Mn = fmaxf(M, mc);
+    const float safe = (Mn == -INFINITY) ? 0.f : Mn;
+    const float c_old = exp2f(M - safe);
+    // weights in parallel (lane p), kept in the record's pad word; L by a warp reduction
+    float lsum = 0.f;
     for (int p = lane; p < n; p += 32) {
-      const float* pp = parts + ((size_t)p * G + hl) * kPartStride;
-      const float mp = __ldcg(pp);
-      const float w = (mp == -INFINITY) ? 0.f : exp2f(mp - mm);
-      sh_w[hl * kCombineMaxParts + p] = w;
-      ls = fmaf(__ldcg(pp + 1), w, ls);
+      const float mp = rec[p * kPartStride];
+      const float w = (mp == -INFINITY) ? 0.f : exp2f(mp - safe);
+      const_cast<float*>(rec)[p * kPartStride + 2] = w;
+      lsum = fmaf(rec[p * kPartStride + 1], w, lsum);
     }
-    ls = warp_sum(ls);
-    if (lane == 0) { sh_L[hl] = ls; sh_M[hl] = mm; }
-  }
-  __syncthreads();
-  float4 acc[G];
-#pragma unroll
-  for (int hl = 0; hl < G; ++hl) acc[hl] = make_float4(0.f, 0.f, 0.f, 0.f);
-  for (int p = warp; p < n; p += kFW) {
-#pragma unroll
-    for (int hl = 0; hl < G; ++hl) {
-      const float w = sh_w[hl * kCombineMaxParts + p];
-      const float4 v = __ldcg(reinterpret_cast<const float4*>(parts + ((size_t)p * G + hl) * kPartStride + 4) + lane);
-      acc[hl].x = fmaf(v.x, w, acc[hl].x); acc[hl].y = fmaf(v.y, w, acc[hl].y);
-      acc[hl].z = fmaf(v.z, w, acc[hl].z); acc[hl].w = fmaf(v.w, w, acc[hl].w);
-    }
-  }
-#pragma unroll
-  for (int hl = 0; hl < G; ++hl) reinterpret_cast<float4*>(sm_o + (warp * G + hl) * kD)[lane] = acc[hl];
-  __syncthreads();
-  for (int o = tid; o < G * kD; o += kFT) {
-    const int hl = o / kD, d = o % kD;
-    float v = 0.f;
-#pragma unroll
-    for (int w = 0; w < kFW; ++w) v += sm_o[(w * G + hl) * kD + d];
-    const float Ls = sh_L[hl];
-    const float res = Ls > 0.f ? v / Ls : 0.f;
-    const size_t oi = ((size_t)b * P.Hq + (size_t)g * G + hl) * kD + d;
-    if (P.out_bf16) reinterpret_cast<__nv_bfloat16*>(P.out)[oi] = __float2bfloat16_rn(res);
-    else reinterpret_cast<float*>(P.out)[oi] = res;
-    if (P.lse && d == 0) P.lse[b * P.Hq + g * G + hl] = Ls > 0.f ? (sh_M[hl] + log2f(Ls)) * kLn2 : -INFINITY;
-  }
-  __syncthreads();
-}
-
-// the partial of an attention item is written; the last item of the group combines
-template <int G>
-__device__ __forceinline__ void attn_item_done(const FusedParams& P, int bg, uint8_t* dsm, Shared& S, float* sm_o) {
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    const int expected = P.bg_part_base[bg + 1] - P.bg_part_base[bg];
-    int* ctr = P.ctrs + 2 + 3 * bg + 1;
-    const int old = atomicAdd(ctr, 1);
-    S.flag = (old == expected - 1);
-    if (S.flag) *ctr = 0;
-  }
-  __syncthreads();
-  if (S.flag) {
-    __threadfence();
-    combine_group<G>(P, bg, dsm, sm_o);
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a3: bitonic sort (descending) of n 64-bit keys in shared memory
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void bitonic_sort_desc(unsigned long long* keys, int n) {
-  for (int size = 2; size <= n; size <<= 1) {
-    for (int stride = size >> 1; stride > 0; stride >>= 1) {
-      for (int i = threadIdx.x; i < (n >> 1); i += kFT) {
-        const int lo = ((i & ~(stride - 1)) << 1) | (i & (stride - 1));
-        const int hi = lo | stride;
-        const bool desc = ((lo & size) == 0);
-        const unsigned long long a = keys[lo], c = keys[hi];
-        if ((a < c) == desc) { keys[lo] = c; keys[hi] = a; }
-      }
-      __syncthreads();
-    }
-  }
-}
-
-// block-wide exclusive scan of one flag per thread; returns this thread's offset, total in *total
-__device__ __forceinline__ int block_scan_flag(bool f, Shared& S, int* total) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned bal = __ballot_sync(0xffffffffu, f);
-  __syncthreads();
-  if (lane == 0) S.scan[warp] = __popc(bal);
-  __syncthreads();
-  int base = 0, tot = 0;
-#pragma unroll
-  for (int w = 0; w < kFW; ++w) { const int c = S.scan[w]; if (w < warp) base += c; tot += c; }
-  *total = tot;
-  return base + __popc(bal & ((1u << lane) - 1u));
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a4: residency plan of (b, g) (one CTA).  The device factor cache of a (layer, sequence, kv head) is
-// `ways` slots with a tag (span id) and a stamp (step of last use).  The first n_zoom entries of
-// sh_ids are this step's zoom set: resident ones are hits, the others are demand misses and take the
-// least-recently-used slots not needed by this step.  Entries n_zoom .. n_cand-1 are prefetch
-// candidates (the next-best spans by routing score): the non-resident ones get a slot too and are
-// copied by the side-stream prefetch kernel after this layer's kernel.  Also: zoom bit-mask for the
-// coarse items (an expanded span's coarse entry is replaced by its tokens),
-// de-duplication of caller-supplied ids, statistics.
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void plan_block(const FusedParams& P, int bg, uint8_t* dsm, Shared& S, int n_zoom, int n_cand,
-                                           bool dedupe, uint32_t epoch) {
-  const int b = bg / P.Hkv, g = bg % P.Hkv, tid = threadIdx.x;
-  const int span0 = P.cv.seq_span_off[b];
-  const int m = P.cv.seq_span_off[b + 1] - span0;
-  const int ways = P.ways;
-  int32_t* sh_ids = reinterpret_cast<int32_t*>(dsm + P.sm_ids);
-  int16_t* way_of = reinterpret_cast<int16_t*>(dsm + P.sm_wayof);
-  int32_t* sh_tag = reinterpret_cast<int32_t*>(dsm + P.sm_tags);
-  uint32_t* sh_stamp = reinterpret_cast<uint32_t*>(sh_tag + ways);
-  int32_t* sh_victim = reinterpret_cast<int32_t*>(sh_stamp + ways);
-  uint32_t* sh_mask = reinterpret_cast<uint32_t*>(dsm + P.sm_mask);
-  int32_t* tags = P.lv.tags + (size_t)bg * ways;
-  uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
-  uint32_t* items = P.lv.items + (size_t)bg * P.kc;
-  int32_t* item_span = P.lv.item_span + (size_t)bg * P.kc;
-  const uint32_t cur = epoch;
-  for (int w = tid; w < P.mask_words; w += kFT) sh_mask[w] = 0u;
-  for (int s = tid; s < m; s += kFT) way_of[s] = (int16_t)-1;
-  for (int w = tid; w < ways; w += kFT) { sh_tag[w] = tags[w]; sh_stamp[w] = stamps[w]; }
-  __syncthreads();
-  for (int w = tid; w < ways; w += kFT) { const int t = sh_tag[w]; if (t >= 0 && t < m) way_of[t] = (int16_t)w; }
-  __syncthreads();
-  unsigned long long n_hit = 0, n_miss = 0, bytes_algo = 0, bytes_h2d = 0, n_pf = 0, bytes_pf = 0;
-  // pass 1: validate / de-duplicate, zoom mask, residency lookup
-  for (int j = tid; j < n_cand; j += kFT) {
-    int id = sh_ids[j];
-    if (id < 0 || id >= m) id = -1;
-    const bool zoom = j < n_zoom;
-    if (id >= 0 && zoom) {
-      const uint32_t bit = 1u << (id & 31);
-      const uint32_t old = atomicOr(&sh_mask[id >> 5], bit);
-      if (dedupe && (old & bit)) id = -1;                      // duplicate of an id seen before: dropped
-    }
-    int way = -1;
-    if (id >= 0) {
-      way = way_of[id];
-      if (way >= 0) sh_stamp[way] = cur;
-      const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + id];
-      const int rk = rr & 0xff, rv = (rr >> 8) & 0xff;
-      const int len = P.cv.span_len[span0 + id];
-      const unsigned long long bb = blob_dims(2, len, rk, rv).bytes;
-      if (zoom) {
-        bytes_algo += (unsigned long long)(rk + rv) * (len + kD) * 2 + 4ull * (rk + rv);
-        if (way >= 0) ++n_hit; else { ++n_miss; bytes_h2d += bb; }
-      } else if (way < 0) { ++n_pf; bytes_pf += bb; }
-    }
-    sh_ids[j] = id;
-    item_span[j] = id;
-    items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
-  }
-  __syncthreads();
-  // victims: ways not used by this step, oldest stamp first (ties to the lower way)
-  for (int w = tid; w < ways; w += kFT) {
-    if (sh_stamp[w] != cur) {
-      int rank = 0;
-      const uint32_t mine = sh_stamp[w];
-      for (int v = 0; v < ways; ++v) {
-        const uint32_t o = sh_stamp[v];
-        rank += (o != cur) && (o < mine || (o == mine && v < w));
-      }
-      sh_victim[rank] = w;
-    }
-  }
-  __syncthreads();
-  // pass 2: misses take victims in item order
-  int miss_base = 0;
-  for (int j0 = 0; j0 < n_cand; j0 += kFT) {
-    const int j = j0 + tid;
-    const bool miss = (j < n_cand) && sh_ids[j] >= 0 && items[j] == 0xFFFFFFFFu;
-    int tot;
-    const int off = block_scan_flag(miss, S, &tot);
-    if (miss) {
-      const int way = sh_victim[miss_base + off];
-      sh_tag[way] = sh_ids[j];
-      sh_stamp[way] = cur;
-      items[j] = (uint32_t)way | 0x80000000u;
-    }
-    miss_base += tot;
-  }
-  __syncthreads();
-  for (int w = tid; w < ways; w += kFT) { tags[w] = sh_tag[w]; stamps[w] = sh_stamp[w]; }
-  uint32_t* gmask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
-  for (int w = tid; w < P.mask_words; w += kFT) gmask[w] = sh_mask[w];
-  if (tid == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
-  // statistics
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    n_hit += __shfl_xor_sync(0xffffffffu, n_hit, o);
-    n_miss += __shfl_xor_sync(0xffffffffu, n_miss, o);
-    bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
-    bytes_h2d += __shfl_xor_sync(0xffffffffu, bytes_h2d, o);
-    n_pf += __shfl_xor_sync(0xffffffffu, n_pf, o);
-    bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
-  }
-  if ((tid & 31) == 0) {
-    if (n_hit) atomicAdd(&P.stats[ST_HITS], n_hit);
-    if (n_miss) atomicAdd(&P.stats[ST_MISSES], n_miss);
-    if (n_hit + n_miss) { atomicAdd(&P.stats[ST_ZOOMED], n_hit + n_miss); atomicAdd(&P.stats[ST_SKIPPED], n_hit + n_miss); }
-    if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
-    if (bytes_h2d + bytes_pf) atomicAdd(&P.stats[ST_H2D], bytes_h2d + bytes_pf);
-    if (n_pf) atomicAdd(&P.stats[ST_PREFETCHED], n_pf);
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) st_release((uint32_t*)(P.ctrs + 2 + 3 * bg + 2), epoch);
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a1-a3: one chunk of spans of (b, g)
-// ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, uint8_t* dsm, Shared& S, uint32_t epoch) {
-  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, tid = threadIdx.x;
-  const int span0 = P.cv.seq_span_off[b];
-  const int m = P.cv.seq_span_off[b + 1] - span0;
-  const int dp = P.dp;
-  unsigned long long* gkeys = P.keys + (size_t)bg * P.sort_n;
-  if (P.mode & FM_ROUTE) {
-    float* sh_q = reinterpret_cast<float*>(dsm);               // [G][128]
-    float* sh_qp = sh_q + G * kD;                              // [G][dp]
-    const __nv_bfloat16* q = P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD;
-    for (int o = tid; o < G * kD; o += kFT) sh_q[o] = __bfloat162float(q[o]);
-    __syncthreads();
-    const __nv_bfloat16* W = (const __nv_bfloat16*)P.lv.W;
-    for (int o = tid; o < G * dp; o += kFT) {                  // Eq. 4: one thread per (head, j)
-      const int hl = o / dp, j = o % dp;
-      const __nv_bfloat16* wr = W + ((size_t)(g * G + hl) * dp + j) * kD;
-      float acc = 0.f;
+    L = fmaf(L, c_old, warp_sum(lsum));
+    acc.x *= c_old; acc.y *= c_old; acc.z *= c_old; acc.w *= c_old;
+    __syncwarp();
 #pragma unroll 4
-      for (int d = 0; d < kD; d += 8) {
-        const uint4 v = *reinterpret_cast<const uint4*>(wr + d);
-        const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          acc = fmaf(__uint_as_float(ww[e] << 16), sh_q[hl * kD + d + 2 * e], acc);
-          acc = fmaf(__uint_as_float(ww[e] & 0xffff0000u), sh_q[hl * kD + d + 2 * e + 1], acc);
-        }
-      }
-      sh_qp[o] = acc;
+    for (int p = 0; p < n; ++p) {
+      const float w = rec[p * kPartStride + 2];
+      const float4 v = reinterpret_cast<const float4*>(rec + p * kPartStride + 4)[lane];
+      acc.x = fmaf(v.x, w, acc.x); acc.y = fmaf(v.y, w, acc.y); acc.z = fmaf(v.z, w, acc.z); acc.w = fmaf(v.w, w, acc.w);
     }
-    __syncthreads();
-    const float inv_sqrt_dp = rsqrtf((float)dp);
-    const __nv_bfloat16* route = (const __nv_bfloat16*)P.lv.route;
-    for (int s = I.a + tid; s < I.b; s += kFT) {
-      const float lnl = P.cv.ln_len[span0 + s];
-      float X = -INFINITY;
-      bool elig = (P.tau == nullptr);
-#pragma unroll
-      for (int hl = 0; hl < G; ++hl) {
-        const int h = g * G + hl;
-        const __nv_bfloat16* kr = route + (size_t)h * P.route_head_stride + (size_t)(span0 + s) * dp;
-        float acc = 0.f;
-        for (int j = 0; j < dp; j += 8) {
-          const uint4 v = ldg16(kr + j);
-          const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            acc = fmaf(__uint_as_float(ww[e] << 16), sh_qp[hl * dp + j + 2 * e], acc);
-            acc = fmaf(__uint_as_float(ww[e] & 0xffff0000u), sh_qp[hl * dp + j + 2 * e + 1], acc);
-          }
-        }
-        const float x = fmaf(acc, inv_sqrt_dp, lnl);           // Eq. 5, pre-sigmoid logit
-        const float a = 1.f / (1.f + __expf(-x));
-        if (P.logits_out) P.logits_out[(size_t)h * P.m_tot + span0 + s] = x;
-        if (P.alpha_out) P.alpha_out[(size_t)h * P.m_tot + span0 + s] = a;
-        if (P.tau != nullptr && a > P.tau[h]) elig = true;     // Eq. 9
-        X = fmaxf(X, x);
-      }
-      gkeys[s] = elig ? (((unsigned long long)order_key(X) << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)s)) : 0ull;
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      int* ctr = P.ctrs + 2 + 3 * bg;
-      const int old = atomicAdd(ctr, 1);
-      S.flag = (old == P.bg_route_items[bg] - 1);
-      if (S.flag) *ctr = 0;
-    }
-    __syncthreads();
-    if (!S.flag) return;
-    __threadfence();
-    // last chunk of the group: top-k
-    unsigned long long* keys = reinterpret_cast<unsigned long long*>(dsm);
-    int my = 0;
-    for (int s = tid; s < P.sort_n; s += kFT) {
-      const unsigned long long k = (s < m) ? __ldcg(gkeys + s) : 0ull;
-      keys[s] = k;
-      my += (k != 0ull);
-    }
-    my = (int)warp_sum((float)my);                 // exact for counts < 2^24
-    __syncthreads();
-    if ((tid & 31) == 0) S.scan[tid >> 5] = my;
-    __syncthreads();
-    int n_elig = 0;
-#pragma unroll
-    for (int w = 0; w < kFW; ++w) n_elig += S.scan[w];
-    bitonic_sort_desc(keys, P.sort_n);
-    int cnt = P.k < 0 ? n_elig : min(P.k, n_elig);
-    cnt = min(cnt, P.k_cap);
-    int n_cand = cnt;
-    if (P.k >= 0 && (P.mode & FM_ATTN)) n_cand = min(min(cnt + P.prefetch, n_elig), P.kc);
-    int32_t* sh_ids = reinterpret_cast<int32_t*>(dsm + P.sm_ids);
-    int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
-    for (int j = tid; j < max(P.k_cap, n_cand); j += kFT) {
-      const int id = j < n_cand ? (int32_t)(0xFFFFFFFFu - (uint32_t)(keys[j] & 0xFFFFFFFFull)) : -1;
-      if (j < n_cand) sh_ids[j] = id;
-      if (j < P.k_cap) my_ids[j] = j < cnt ? id : -1;
-    }
-    if (tid == 0) P.count[bg] = cnt;
-    __syncthreads();
-    if (P.mode & FM_ATTN) plan_block(P, bg, dsm, S, cnt, n_cand, false, epoch);
-  } else {
-    // caller-supplied zoom set (sekv_decode_attn): the group's first chunk item runs the plan
-    if (I.a != 0) return;
-    int cnt = 0;
-    if (P.ids != nullptr && P.count != nullptr) cnt = max(0, min(P.count[bg], P.k_cap));
-    int32_t* sh_ids = reinterpret_cast<int32_t*>(dsm + P.sm_ids);
-    const int32_t* src = P.ids + (size_t)bg * max(P.k_cap, 1);
-    for (int j = tid; j < cnt; j += kFT) sh_ids[j] = src[j];
-    __syncthreads();
-    plan_block(P, bg, dsm, S, cnt, cnt, true, epoch);
+    M = Mn;
   }
+  const float inv = L > 0.f ? 1.f / L : 0.f;
+  const size_t oi = ((size_t)b * P.Hq + (size_t)g * G + hl) * kD + 4 * lane;
+  if (P.out_bf16) {
+    uint2 o;
+    o.x = pack_bf16(acc.x * inv, acc.y * inv);
+    o.y = pack_bf16(acc.z * inv, acc.w * inv);
+    *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(P.out) + oi) = o;
+  } else {
+    *reinterpret_cast<float4*>(reinterpret_cast<float*>(P.out) + oi) = make_float4(acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv);
+  }
+  if (P.lse && lane == 0) P.lse[b * P.Hq + g * G + hl] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
+}
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+
+__device__ __forceinline__ Item load_item(const Item* p) {
+  const uint4* s = reinterpret_cast<const uint4*>(p);
+  const uint4 a = __ldg(s), c = __ldg(s + 1), d = __ldg(s + 2);
+  Item I;
+  I.kind = (int32_t)a.x; I.bg = (int32_t)a.y; I.a = (int32_t)a.z; I.b = (int32_t)a.w;
+  I.part = (int32_t)c.x; I.A = (int32_t)c.y; I.row0 = (int32_t)c.z; I.span0 = (int32_t)c.w;
+  I.pbase = (int32_t)d.x; I.np = (int32_t)d.y; I.pad0 = 0; I.pad1 = 0;
+  return I;
 }
 
 template <int G>
-__global__ void __launch_bounds__(kFT, 3) fused_layer_kernel(const __grid_constant__ FusedParams P) {
+__global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_constant__ FusedParams P) {
   extern __shared__ __align__(128) uint8_t dsm[];
-  __shared__ Shared S;
-  __shared__ __align__(16) float sm_o[kFW * G * kD];
-  const int tid = threadIdx.x;
+  __shared__ uint64_t bars[8];
+  __shared__ int last_flag;
+  __shared__ unsigned long long tmid_s[8 * 4];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+  uint8_t* region = dsm + (size_t)warp * P.region_bytes;
+  uint64_t* bar = &bars[warp];
   const uint32_t epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
-  if (tid == 0) {
-    mbar_init(&S.bars[0], 1);
-    mbar_init(&S.bars[1], 1);
+  if (lane == 0) {
+    mbar_init(bar, 1);
     mbar_fence_init();
   }
-  __syncthreads();
-  uint32_t phase[2] = {0u, 0u};
-  for (;;) {
-    if (tid == 0) S.item = atomicAdd(P.ctrs, 1);
-    __syncthreads();
-    const int it = S.item;
-    __syncthreads();
-    if (it >= P.n_items) break;
-    const Item I = P.items[it];
-    if (I.kind == IT_ROUTE) {
-      route_item<G>(P, I, dsm, S, epoch);
-      __syncthreads();
-      continue;
+  __syncwarp();
+  uint32_t phase = 0u;
+  unsigned long long* tm = P.trace ? &tmid_s[warp * 4] : nullptr;
+
+  // even warps start on the latency queue, odd warps on the main queue; first item static
+  const int nlw = (nw + 1) >> 1, nmw = nw >> 1;
+  const int total_lw = (int)gridDim.x * nlw, total_mw = (int)gridDim.x * nmw;
+  bool in_lat = (warp & 1) == 0;
+  auto claim = [&]() -> int {
+    int i = 0;
+    if (in_lat) {
+      if (lane == 0) i = P.lat_begin + total_lw + atomicAdd(P.ctrs, 1);
+      i = __shfl_sync(0xffffffffu, i, 0);
+      if (i < P.lat_end) return i;
+      in_lat = false;
     }
-    float* part = P.partials + ((size_t)P.bg_part_base[I.bg] + I.part) * G * kPartStride;
-    if (I.kind == IT_POOL) {
-      rows_item<G>(P, I.bg, I.a, I.b, sm_o, S.ml, part);
-    } else if (I.kind == IT_COARSE) {
-      wait_plan(P, I.bg, epoch);
-      rows_item<G>(P, I.bg, I.a, I.b, sm_o, S.ml, part);
-    } else {
-      wait_plan(P, I.bg, epoch);
-      zoom_item<G>(P, I, dsm, S, sm_o, phase, part);
-    }
-    attn_item_done<G>(P, I.bg, dsm, S, sm_o);
+    if (lane == 0) i = P.lat_end + total_mw + atomicAdd(P.ctrs + 1, 1);
+    return __shfl_sync(0xffffffffu, i, 0);
+  };
+  int idx;
+  if (in_lat) {
+    idx = P.lat_begin + (int)blockIdx.x * nlw + (warp >> 1);
+    if (idx >= P.lat_end) { in_lat = false; idx = claim(); }
+  } else {
+    idx = P.lat_end + (int)blockIdx.x * nmw + (warp >> 1);
   }
-  // last CTA out re-arms the queue and advances the layer's step stamp
+  if (idx < P.main_end) {
+    // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular): the
+    // item after a POOL item is claimed, and its descriptor loaded, while the POOL item is processed.  Any
+    // other item is claimed when the warp is free to run it, so it never waits behind a slow item.
+    auto claim_after = [&](int just) -> int { return (!in_lat && just < P.pool_end) ? claim() : -1; };
+    Item cur = load_item(P.items + idx);
+    int nidx = claim_after(idx);
+    for (;;) {
+      const bool has_next = nidx >= 0 && nidx < P.main_end;
+      Item nxt = cur;
+      int nnidx = nidx;
+      if (has_next) {
+        nxt = load_item(P.items + nidx);
+        nnidx = claim_after(nidx);
+      }
+      unsigned long long t0 = 0ull;
+      const int cur_idx = idx;
+      if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
+      switch (cur.kind) {
+        case IT_QPROJ: qproj_item(P, cur, lane); break;
+        case IT_ROUTE: route_item(P, cur, region, lane, tm); break;
+        case IT_SELECT: select_item(P, cur, region, lane, epoch, tm); break;
+        case IT_POOL:
+        case IT_COARSE: rows_item<G>(P, cur, region, lane, tm); break;
+        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, tm); break;
+        default: combine_item(P, cur, region, bar, phase, lane, tm); break;
+      }
+      if (P.trace && lane == 0 && cur_idx < P.trace_cap) {
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        unsigned long long* r = P.trace + 8 * (size_t)cur_idx;
+        r[0] = (unsigned long long)(uint32_t)cur.kind | ((unsigned long long)(uint32_t)cur.bg << 32);
+        r[1] = (unsigned long long)(smid & 0xffffu) | ((unsigned long long)(uint32_t)warp << 16);
+        r[2] = t0; r[3] = globaltimer_ns();
+        r[4] = tm[0]; r[5] = tm[1]; r[6] = tm[2]; r[7] = tm[3];
+      }
+      if (nidx < 0) {
+        nidx = claim();
+        if (nidx >= P.main_end) break;
+        cur = load_item(P.items + nidx);
+        idx = nidx;
+        nidx = claim_after(idx);
+        continue;
+      }
+      if (!has_next) break;
+      cur = nxt;
+      idx = nidx;
+      nidx = nnidx;
+    }
+  }
+  // last CTA out re-arms the queues and counters and advances the layer's step stamp
+  __syncthreads();
   if (tid == 0) {
     __threadfence();
-    const int old = atomicAdd(P.ctrs + 1, 1);
-    if (old == (int)gridDim.x - 1) {
-      P.ctrs[0] = 0;
-      P.ctrs[1] = 0;
-      if (P.mode & FM_ATTN) {
-        *P.lv.layer_step = epoch;
-        atomicAdd(&P.stats[ST_LAYER_STEPS], 1ull);
-      }
-      __threadfence();
+    const int old = atomicAdd(P.ctrs + 2, 1);
+    last_flag = (old == (int)gridDim.x - 1);
+  }
+  __syncthreads();
+  if (last_flag) {
+    __threadfence();
+    for (int i = tid; i < 4 + 4 * P.BG; i += blockDim.x) P.ctrs[i] = 0;
+    if (tid == 0 && (P.mode & FM_ATTN)) {
+      *P.lv.layer_step = epoch;
+      atomicAdd(&P.stats[ST_LAYER_STEPS], 1ull);
     }
   }
 }
@@ -869,9 +1063,9 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
   if (j >= plan_counts[2 * bg + 1]) return;
   const int id = lv.item_span[(size_t)bg * kc + j];
   const uint32_t it = lv.items[(size_t)bg * kc + j];
-  if (id < 0 || !(it & 0x80000000u)) return;
+  if (id < 0 || (it & 0xC0000000u) != 0x80000000u) return;
   if (threadIdx.x == 0) {
-    const int way = (int)(it & 0x7FFFFFFFu);
+    const int way = (int)(it & 0x3FFFFFFFu);
     const int gs = cv.seq_span_off[b] + id;
     const int rr = lv.dir_rank[(size_t)g * spans_cap + gs];
     const uint32_t bytes = (uint32_t)blob_dims(2, cv.span_len[gs], rr & 0xff, (rr >> 8) & 0xff).bytes;
@@ -892,10 +1086,15 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
 // ---------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------
+static int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+// byte offsets of the select / plan tables inside a warp's region; returns the bytes they need
 size_t fused_plan_smem(const sekv_handle* h, FusedParams* P) {
   const sekv_config& c = h->cfg;
   const int kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
-  size_t o = (size_t)h->sort_n * 8;
+  size_t o = (size_t)round_up(std::max(h->max_m, 1), 4) * 4;             // keys
+  o = round_up_sz(o, 16); P->sm_hist = (int)o; o += 256 * 4;
+  o = round_up_sz(o, 16); P->sm_cand = (int)o; o += (size_t)pow2_ceil(std::max(kc, 64)) * 8;
   o = round_up_sz(o, 16); P->sm_ids = (int)o; o += (size_t)kc * 4;
   o = round_up_sz(o, 16); P->sm_wayof = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 8) * 2;
   o = round_up_sz(o, 16); P->sm_tags = (int)o; o += (size_t)c.cache_ways * 12;
@@ -903,48 +1102,40 @@ size_t fused_plan_smem(const sekv_handle* h, FusedParams* P) {
   return o;
 }
 
+// per-warp region: the rows ring, one factor blob, or the select / plan tables
+size_t fused_region_bytes(const sekv_handle* h, FusedParams* P) {
+  FusedParams tmp;
+  if (!P) P = &tmp;
+  size_t need = fused_plan_smem(h, P);
+  need = std::max(need, (size_t)kStages * kStageBytes);
+  if (h->cfg.k_cap > 0) need = std::max(need, (size_t)h->lay.slot_bytes);
+  need = std::max(need, (size_t)kPartStride * 4 * 8);
+  return round_up_sz(need, 128);
+}
+
+// spans per ROUTE item: their G x dp rows plus q' fit the smallest region
+int fused_route_spans(const sekv_handle* h) {
+  const int per_span = h->G * h->cfg.route_dim * 2;
+  const int cap = (kStages * kStageBytes - h->G * h->cfg.route_dim * 4) / per_span;
+  return std::max(8, std::min(64, cap / 8 * 8));
+}
+
+int fused_warps(const sekv_handle* h) {
+  const size_t region = fused_region_bytes(h, nullptr);
+  const size_t budget = 227 * 1024 - 1024;
+  return (int)std::min<size_t>(8, budget / region);
+}
+
 template <int G>
-static cudaError_t launch_fused_g(sekv_handle* h, const FusedParams& P, size_t smem, int grid, cudaStream_t s) {
+static cudaError_t launch_fused_g(const FusedParams& P, size_t smem, int grid, int threads, cudaStream_t s) {
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  fused_layer_kernel<G><<<grid, kFT, smem, s>>>(P);
+  fused_layer_kernel<G><<<grid, threads, smem, s>>>(P);
   return cudaGetLastError();
-}
-
-template <int G>
-static int fused_occupancy_g(size_t smem) {
-  int n = 0;
-  cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_layer_kernel<G>, kFT, smem);
-  return n;
-}
-
-size_t fused_smem_bytes(const sekv_handle* h, FusedParams* P) {
-  const sekv_config& c = h->cfg;
-  FusedParams tmp;
-  if (!P) P = &tmp;
-  size_t need = fused_plan_smem(h, P);
-  const size_t slotp = round_up_sz((size_t)h->lay.slot_bytes, 128);
-  P->smem_buf_stride = (int64_t)slotp;
-  if (c.k_cap > 0) need = std::max(need, 2 * slotp);
-  need = std::max(need, (size_t)(h->G * kCombineMaxParts + 2 * SEKV_MAX_GROUP) * 4);
-  need = std::max(need, (size_t)h->G * (kD + c.route_dim) * 4);
-  return round_up_sz(need, 128);
-}
-
-int fused_occupancy(const sekv_handle* h) {
-  const size_t smem = fused_smem_bytes(h, nullptr);
-  switch (h->G) {
-    case 1: return fused_occupancy_g<1>(smem); case 2: return fused_occupancy_g<2>(smem);
-    case 3: return fused_occupancy_g<3>(smem); case 4: return fused_occupancy_g<4>(smem);
-    case 5: return fused_occupancy_g<5>(smem); case 6: return fused_occupancy_g<6>(smem);
-    case 7: return fused_occupancy_g<7>(smem); case 8: return fused_occupancy_g<8>(smem);
-  }
-  return 0;
 }
 
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
@@ -957,35 +1148,43 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.q = (const __nv_bfloat16*)q; P.tau = tau; P.logits_out = logits; P.alpha_out = alpha;
   P.ids = ids; P.count = count; P.out = out; P.lse = lse;
   P.items = (const Item*)ws(h, h->F.off_items_sched);
-  P.n_items = (mode & FM_ATTN) ? h->n_items : h->n_route_items;
-  P.bg_part_base = (const int32_t*)ws(h, h->F.off_bg_part);
-  P.bg_route_items = (const int32_t*)ws(h, h->F.off_bg_route);
   P.partials = (float*)ws(h, h->F.off_partials1);
-  P.keys = (unsigned long long*)ws(h, h->F.off_keys);
+  P.keys = (uint32_t*)ws(h, h->F.off_keys);
+  P.qp = (float*)ws(h, h->F.off_qp);
+  P.zdesc = (ZDescG*)ws(h, h->F.off_zdesc);
   P.ctrs = (int32_t*)ws(h, h->F.off_ctrs) + (size_t)layer * h->F.ctrs_per_layer;
   P.plan_counts = (int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
   P.stats = (unsigned long long*)ws(h, h->F.off_stats);
   P.host_arena = h->host_dev;
+  P.trace = (unsigned long long*)h->trace_buf; P.trace_cap = h->trace_cap;
   P.mode = mode; P.k = k; P.k_cap = c.k_cap; P.prefetch = std::max(c.prefetch, 0);
   P.kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
+  P.BG = h->n_seqs * c.n_kv_heads;
   P.Hq = c.n_q_heads; P.Hkv = c.n_kv_heads; P.dp = c.route_dim; P.ways = c.cache_ways;
-  P.mask_words = h->mask_words; P.spans_cap = (int)h->lay.spans_cap; P.m_tot = h->m_tot; P.sort_n = h->sort_n;
+  P.mask_words = h->mask_words; P.spans_cap = (int)h->lay.spans_cap; P.m_tot = h->m_tot; P.keys_stride = h->F.keys_per_bg;
   P.out_bf16 = c.out_dtype == SEKV_BF16;
   P.slot_bytes = h->lay.slot_bytes;
   P.ent_head_stride = (size_t)h->lay.rows_cap * kD;
   P.route_head_stride = (size_t)h->lay.spans_cap * c.route_dim;
-  const size_t smem = fused_smem_bytes(h, &P);
-  const int grid = std::max(1, std::min(P.n_items, h->fused_grid));
+  P.region_bytes = (int)fused_region_bytes(h, &P);
+  P.route_spans = fused_route_spans(h);
+  // queues: [QPROJ, ROUTE | SELECT | POOL, ZOOM, COARSE, COMBINE]
+  P.pool_end = h->pool_end;
+  if (mode == FM_ROUTE) { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_lat_items; }
+  else if (mode == FM_ATTN) { P.lat_begin = h->select_begin; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }
+  else { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }
+  const size_t smem = (size_t)h->fused_warps * P.region_bytes;
+  const int grid = h->fused_grid, threads = 32 * h->fused_warps;
   cudaError_t e;
   switch (h->G) {
-    case 1: e = launch_fused_g<1>(h, P, smem, grid, s); break;
-    case 2: e = launch_fused_g<2>(h, P, smem, grid, s); break;
-    case 3: e = launch_fused_g<3>(h, P, smem, grid, s); break;
-    case 4: e = launch_fused_g<4>(h, P, smem, grid, s); break;
-    case 5: e = launch_fused_g<5>(h, P, smem, grid, s); break;
-    case 6: e = launch_fused_g<6>(h, P, smem, grid, s); break;
-    case 7: e = launch_fused_g<7>(h, P, smem, grid, s); break;
-    case 8: e = launch_fused_g<8>(h, P, smem, grid, s); break;
+    case 1: e = launch_fused_g<1>(P, smem, grid, threads, s); break;
+    case 2: e = launch_fused_g<2>(P, smem, grid, threads, s); break;
+    case 3: e = launch_fused_g<3>(P, smem, grid, threads, s); break;
+    case 4: e = launch_fused_g<4>(P, smem, grid, threads, s); break;
+    case 5: e = launch_fused_g<5>(P, smem, grid, threads, s); break;
+    case 6: e = launch_fused_g<6>(P, smem, grid, threads, s); break;
+    case 7: e = launch_fused_g<7>(P, smem, grid, threads, s); break;
+    case 8: e = launch_fused_g<8>(P, smem, grid, threads, s); break;
     default: return cudaErrorInvalidValue;
   }
   h->launches += 1;

@@ -89,11 +89,11 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   L.slot_bytes = (int64_t)bd.bytes;
   L.cache_slots = cv.take((size_t)regions * c.cache_ways * bd.bytes);
   // workspace
-  // capacity of the stage-1 chunk list (generic path) and of the fused kernel's item list
-  const int64_t zs_min = std::max<int64_t>(1, c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 4);
-  const int64_t attn_items = Hkv * (rcap / 64 + 2 * B + 2) + B * Hkv * ((kcap + zs_min - 1) / zs_min);
+  // capacity of the stage-1 chunk list (generic path) and of the fused kernel's item list (row items of
+  // >= 16 rows, one expanded span per ZOOM item at the finest)
+  const int64_t attn_items = Hkv * (rcap / 16 + 2 * B + 2) + B * Hkv * kcap;
   F->max_chunks = (int)std::max<int64_t>(std::max(c.stage1_ctas, 1024) + B * Hkv, attn_items);
-  F->max_items = (int)(attn_items + Hkv * (mcap / 256 + B + 1));
+  F->max_items = (int)(attn_items + 2 * B * Hq + B * Hkv + Hkv * (mcap / 8 + B + 1));
   const int G = c.n_q_heads / c.n_kv_heads;
   const int P2 = (kcap + kStage2SpansPerCta - 1) / kStage2SpansPerCta;
   F->off_partials1 = cv.take((size_t)F->max_chunks * G * kPartStride * 4);
@@ -114,7 +114,9 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   while (kpb < std::min<int64_t>(mcap, SEKV_MAX_SPANS_PER_SEQ)) kpb <<= 1;
   F->keys_per_bg = kpb;
   F->off_keys = cv.take((size_t)B * Hkv * kpb * 8);
-  F->ctrs_per_layer = (int)(2 + 3 * B * Hkv);
+  F->ctrs_per_layer = (int)(4 + 4 * B * Hkv);
+  F->off_qp = cv.take((size_t)B * Hq * c.route_dim * 4);
+  F->off_zdesc = cv.take((size_t)B * Hkv * kc * sizeof(ZDescG));
   F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);
   F->off_plan_counts = cv.take((size_t)NL * B * Hkv * 2 * 4);
   F->off_layer_step = cv.take((size_t)NL * 4);
@@ -266,6 +268,7 @@ sekv_status sekv_create(const sekv_config* cfg, void* device_arena, size_t devic
   cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
   h->launches = 0;
   h->profiling = false;
+  h->trace_buf = nullptr; h->trace_cap = 0;
   *out = h;
   sekv_status s = sekv_reset(h);
   if (s != SEKV_OK) { sekv_destroy(h); *out = nullptr; return s; }
@@ -305,7 +308,7 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
-  h->n_items = h->n_route_items = 0; h->use_fused = false;
+  h->n_items = h->n_lat_items = h->select_begin = 0; h->use_fused = false;
   h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
   h->span_len_host.clear();
   h->m_tot = h->A_tot = h->max_m = 0;
@@ -384,75 +387,92 @@ static sekv_status make_schedule(sekv_handle* h) {
   return SEKV_OK;
 }
 
-// Work-item list of the fused layer kernel (bf16 path), in queue order: ROUTE chunks, POOL row ranges,
-// ZOOM item ranges, COARSE row ranges.  A topological order: ZOOM / COARSE items depend on the plan that the
-// last ROUTE chunk of their (sequence, kv head) publishes.
+// Work-item lists of the fused layer kernel (bf16 path), in queue order.  Latency queue: QPROJ, ROUTE,
+// SELECT; main queue: POOL, ZOOM, COARSE, COMBINE.  Both are topological orders of the dependencies
+// (ROUTE after QPROJ, SELECT after ROUTE, ZOOM / COARSE after SELECT, COMBINE after the attention items).
 static sekv_status make_fused_schedule(sekv_handle* h) {
   const FullLayout& F = h->F;
   const sekv_config& c = h->cfg;
   h->use_fused = false;
   if (c.dtype != SEKV_BF16 || c.impl == 1) return SEKV_OK;
-  const int B = h->n_seqs, Hkv = c.n_kv_heads, BG = B * Hkv;
-  if (h->max_m > SEKV_MAX_SPANS_PER_SEQ) return SEKV_OK;
-  const size_t smem = fused_smem_bytes(h, nullptr);
-  if (smem + 20 * 1024 > 227 * 1024) return SEKV_OK;        // blobs too large to double-buffer: generic path
-  int occ = fused_occupancy(h);
-  cudaGetLastError();
-  if (occ < 1) return SEKV_OK;
-  h->fused_occ = occ;
-  h->fused_grid = occ * h->num_sms;
-  long total_rows = 0;
-  int max_rows = 0;
-  for (int b = 0; b < B; ++b) { total_rows += (long)(h->A_b[b] + h->m_b[b]) * Hkv; max_rows = std::max(max_rows, h->A_b[b] + h->m_b[b]); }
-  int rows = c.item_rows;
-  if (rows <= 0) {
-    rows = (int)((total_rows * 2 + 5L * h->fused_grid - 1) / (5L * h->fused_grid));     // ~2.5 items per resident CTA
-    rows = std::min(256, std::max(64, round_up(rows, 64)));
-  }
-  rows = std::max(rows, round_up((max_rows + 299) / 300, 16));                           // <= ~300 row items per group
+  const int B = h->n_seqs, Hkv = c.n_kv_heads, BG = B * Hkv, G = h->G;
+  if (h->max_m > 2048) return SEKV_OK;                      // select / plan tables live in one warp's region
+  if (c.route_dim != 8 && c.route_dim != 16 && c.route_dim != 32 && c.route_dim != 64) return SEKV_OK;
+  const int nw = fused_warps(h);
+  if (nw < 1) return SEKV_OK;                               // blobs too large for shared memory: generic path
+  h->fused_warps = nw;
+  h->fused_grid = h->num_sms;                               // one resident CTA per SM
+  int rows = c.item_rows > 0 ? c.item_rows : 64;
   h->fused_item_rows = rows;
-  const int kcap = std::max(c.k_cap, 1);
-  int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 4;
-  zs = std::max(zs, (kcap + 127) / 128);                                                  // <= 128 zoom items per group
+  const int crows = std::min(rows, 64);
+  int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 1;
+  const int rspans = fused_route_spans(h);
   std::vector<Item> items;
-  std::vector<int32_t> part_base(BG + 1, 0), route_items(BG, 0), nparts(BG, 0);
+  std::vector<int32_t> nparts(BG, 0), pbase(BG, 0);
+  auto mk = [&](int kind, int b, int g, int a, int bb, int part) {
+    Item it;
+    memset(&it, 0, sizeof(it));
+    it.kind = kind; it.bg = b * Hkv + g; it.a = a; it.b = bb; it.part = part;
+    it.A = h->A_b[b]; it.row0 = 0; it.span0 = 0;
+    for (int s = 0; s < b; ++s) { it.row0 += h->A_b[s] + h->m_b[s]; it.span0 += h->m_b[s]; }
+    return it;
+  };
+  // partial slots first (attention items need np of their group)
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g) {
-      const int bg = b * Hkv + g, m = h->m_b[b];
-      int n = 0;
-      for (int s0 = 0; s0 == 0 || s0 < m; s0 += 256, ++n) items.push_back(Item{IT_ROUTE, bg, s0, std::min(m, s0 + 256), 0});
-      route_items[bg] = n;
+      const int A = h->A_b[b], m = h->m_b[b];
+      int n = (A + rows - 1) / rows + (m + crows - 1) / crows;
+      if (c.k_cap > 0) n += (std::min(c.k_cap, m) + zs - 1) / zs;
+      nparts[b * Hkv + g] = n;
     }
-  h->n_route_items = (int)items.size();
+  int total_parts = 0;
+  for (int bg = 0; bg < BG; ++bg) { pbase[bg] = total_parts * G; total_parts += nparts[bg]; }
+  if (total_parts > F.max_chunks) return SEKV_OK;
+  std::vector<int32_t> next_part(BG, 0);
+  auto attn = [&](int kind, int b, int g, int a, int bb) {
+    const int bg = b * Hkv + g;
+    Item it = mk(kind, b, g, a, bb, next_part[bg]++);
+    it.pbase = pbase[bg]; it.np = nparts[bg];
+    items.push_back(it);
+  };
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g)
+      for (int hl = 0; hl < G; ++hl) items.push_back(mk(IT_QPROJ, b, g, hl, 0, 0));
+  std::vector<int32_t> route_items(BG, 0);
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g) {
-      const int bg = b * Hkv + g, A = h->A_b[b];
-      for (int r0 = 0; r0 < A; r0 += rows) items.push_back(Item{IT_POOL, bg, r0, std::min(A, r0 + rows), nparts[bg]++});
+      const int m = h->m_b[b];
+      for (int s0 = 0; s0 < m; s0 += rspans) { items.push_back(mk(IT_ROUTE, b, g, s0, std::min(m, s0 + rspans), 0)); ++route_items[b * Hkv + g]; }
     }
+  h->select_begin = (int)items.size();
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) items.push_back(mk(IT_SELECT, b, g, route_items[b * Hkv + g], h->m_b[b], 0));
+  h->n_lat_items = (int)items.size();
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g)
+      for (int r0 = 0; r0 < h->A_b[b]; r0 += rows) attn(IT_POOL, b, g, r0, std::min(h->A_b[b], r0 + rows));
+  h->pool_end = (int)items.size();
   if (c.k_cap > 0)
     for (int b = 0; b < B; ++b)
       for (int g = 0; g < Hkv; ++g) {
-        const int bg = b * Hkv + g;
         const int kmax = std::min(c.k_cap, h->m_b[b]);
-        for (int j0 = 0; j0 < kmax; j0 += zs) items.push_back(Item{IT_ZOOM, bg, j0, std::min(kmax, j0 + zs), nparts[bg]++});
+        for (int j0 = 0; j0 < kmax; j0 += zs) attn(IT_ZOOM, b, g, j0, std::min(kmax, j0 + zs));
       }
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g) {
-      const int bg = b * Hkv + g, A = h->A_b[b], R = h->A_b[b] + h->m_b[b];
-      for (int r0 = A; r0 < R; r0 += rows) items.push_back(Item{IT_COARSE, bg, r0, std::min(R, r0 + rows), nparts[bg]++});
+      const int A = h->A_b[b], R = A + h->m_b[b];
+      for (int r0 = A; r0 < R; r0 += crows) attn(IT_COARSE, b, g, r0, std::min(R, r0 + crows));
     }
-  int total_parts = 0;
-  for (int bg = 0; bg < BG; ++bg) {
-    part_base[bg] = total_parts;
-    total_parts += nparts[bg];
-    if (nparts[bg] > 512 || nparts[bg] < 1) return SEKV_OK;                               // combine capacity: generic path
-  }
-  part_base[BG] = total_parts;
-  if ((int)items.size() > F.max_items || total_parts > F.max_chunks) return SEKV_OK;
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g)
+      for (int hl = 0; hl < G; ++hl) {
+        Item it = mk(IT_COMBINE, b, g, hl, 0, 0);
+        it.pbase = pbase[b * Hkv + g]; it.np = nparts[b * Hkv + g];
+        items.push_back(it);
+      }
+  if ((int)items.size() > F.max_items) return SEKV_OK;
   h->n_items = (int)items.size();
   CK(h, cudaMemcpyAsync(h->dev + F.off_items_sched, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice, h->main));
-  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_part, part_base.data(), part_base.size() * 4, cudaMemcpyHostToDevice, h->main));
-  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_route, route_items.data(), route_items.size() * 4, cudaMemcpyHostToDevice, h->main));
   CK(h, cudaStreamSynchronize(h->main));
   h->use_fused = true;
   return SEKV_OK;
@@ -879,6 +899,17 @@ sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t* launches
   }
   cudaGetLastError();
   prof_clear(h);
+  return SEKV_OK;
+}
+
+sekv_status sekv_set_trace(sekv_handle* h, void* buf, int64_t capacity_items, int32_t* n_items) {
+  if (!h) return SEKV_INVALID_ARG;
+  CK(h, cudaStreamSynchronize(h->main));
+  h->trace_buf = buf;
+  h->trace_cap = buf ? capacity_items : 0;
+  for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);     // captured launches carry the old pointer
+  h->graphs.clear();
+  if (n_items) *n_items = h->n_items;
   return SEKV_OK;
 }
 

@@ -103,13 +103,33 @@ struct Chunk {  // one stage-1 work item
 enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_PREFETCHED, ST_COUNT = 8 };
 
 // ---- fused layer kernel (fused_kernels.cu) -------------------------------------------------------
-enum ItemKind { IT_ROUTE = 0, IT_POOL = 1, IT_ZOOM = 2, IT_COARSE = 3 };
+// Work items of the per-layer persistent kernel.  Every item is processed by ONE warp.  Two queues:
+//   latency queue : QPROJ (Eq. 4), ROUTE (Eq. 5), SELECT (Eq. 9 top-k + factor-cache plan)
+//   main queue    : POOL, ZOOM, COARSE (L119-121, Eq. 8), COMBINE (L61)
+enum ItemKind { IT_QPROJ = 0, IT_ROUTE = 1, IT_SELECT = 2, IT_POOL = 3, IT_ZOOM = 4, IT_COARSE = 5, IT_COMBINE = 6 };
 enum FusedMode { FM_ROUTE = 1, FM_ATTN = 2 };   // FM_ATTN without FM_ROUTE: caller-supplied zoom set
-struct Item {          // one work item of the layer kernel's queue
+struct __align__(16) Item {   // 48 bytes: three 16-byte loads
   int32_t kind;        // ItemKind
   int32_t bg;          // b * H_kv + g
-  int32_t a, b;        // ROUTE: span range; POOL / COARSE: entry-row range; ZOOM: plan-item range
+  int32_t a, b;        // QPROJ/COMBINE: a = head within the group; ROUTE: span range; SELECT: a = route items of
+                       // the group, b = m; POOL / COARSE: entry-row range; ZOOM: plan-item range
   int32_t part;        // partial slot within the group (attention items)
+  int32_t A;           // pool rows of the sequence
+  int32_t row0;        // first entry row of the sequence
+  int32_t span0;       // first span of the sequence
+  int32_t pbase;       // first partial record of the group (records of kPartStride floats)
+  int32_t np;          // partials per head of the group
+  int32_t pad0, pad1;
+};
+
+struct __align__(16) ZDescG {   // what a ZOOM item needs to know about one expanded span (written by the plan)
+  unsigned long long src;       // blob address: cache slot (hit) or device alias of the pinned-host store (miss)
+  uint32_t bytes;
+  int32_t len;
+  int32_t rr;                   // rank_k | rank_v << 8
+  uint32_t way_miss;            // way | miss << 31
+  int32_t id;                   // local span id, -1 = dropped duplicate
+  int32_t pad;
 };
 
 struct FusedParams {
@@ -124,19 +144,25 @@ struct FusedParams {
   void* out;                   // [B][H][128]
   float* lse;                  // [B][H] or null
   const Item* items;
-  const int32_t* bg_part_base;   // [BG+1] first partial of each group
-  const int32_t* bg_route_items; // [BG]   route chunk items per group
-  float* partials;
-  unsigned long long* keys;    // [BG][sort_n]
-  int32_t* ctrs;               // [0] queue, [1] exited CTAs, then per group: route_done, attn_done, plan_flag
+  float* partials;             // records [pbase + hl * np + part][kPartStride]
+  uint32_t* keys;              // [BG][keys_stride] ordered routing keys (0 = not eligible)
+  float* qp;                   // [BG][G][dp] projected queries
+  ZDescG* zdesc;               // [BG][kc]
+  int32_t* ctrs;               // [0] latency queue, [1] main queue, [2] exited CTAs, [3] pad, then per group:
+                               // qp_done, route_done, attn_done, plan_flag
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
   unsigned long long* stats;
   const uint8_t* host_arena;   // device alias of the pinned host factor store
+  unsigned long long* trace;   // null, or 4 x u64 per item (sekv_set_trace)
   size_t ent_head_stride, route_head_stride;
-  int64_t slot_bytes, smem_buf_stride;
-  int32_t n_items, mode, k, k_cap, prefetch, kc;
-  int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, sort_n, out_bf16;
-  int32_t sm_ids, sm_wayof, sm_tags, sm_mask;   // byte offsets in dynamic shared memory (plan)
+  int64_t slot_bytes, trace_cap;
+  int32_t lat_begin, lat_end, main_end;         // item index ranges of the two queues
+  int32_t pool_end;                              // first main-queue item that is not a POOL item
+  int32_t mode, k, k_cap, prefetch, kc, BG;
+  int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, keys_stride, out_bf16;
+  int32_t region_bytes;                          // per-warp shared-memory region
+  int32_t route_spans;                           // spans per ROUTE item
+  int32_t sm_cand, sm_ids, sm_wayof, sm_tags, sm_mask, sm_hist;   // byte offsets in the region (select / plan)
 };
 
 // ---- storage-type helpers ------------------------------------------------------------------------
@@ -193,7 +219,7 @@ struct FullLayout {
   int64_t off_partials1, off_partials2, off_ws_ids, off_ws_count, off_stats, off_chunks, off_bg_chunk,
       off_zoom_mask, off_items, off_item_span, off_layer_step, off_seg_flag, off_seg_flag2, off_seg_len,
       off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag, off_items_sched, off_bg_part,
-      off_bg_route, off_keys, off_ctrs, off_plan_counts;
+      off_bg_route, off_keys, off_ctrs, off_plan_counts, off_qp, off_zdesc;
   int mask_words, max_chunks, max_items, ctrs_per_layer, keys_per_bg;
   size_t total;
 };
@@ -223,12 +249,13 @@ struct sekv_handle {
   int n_chunks, parts1_max, P2, parts_per_head, sort_n;
   // fused layer kernel (bf16 path)
   bool use_fused;
-  int n_items, n_route_items, fused_grid, fused_occ, fused_item_rows;
+  int n_items, n_lat_items, select_begin, pool_end, fused_grid, fused_warps, fused_item_rows;
   int num_sms;
   std::vector<GraphEntry> graphs;
   uint64_t launches;
   // per-kernel-class CUDA-event timing (sekv_set_profiling)
   bool profiling;
+  void* trace_buf; int64_t trace_cap;
   struct ProfRec { int cls; cudaEvent_t a, b; };
   std::vector<ProfRec> prof;
   std::string err;
@@ -267,8 +294,9 @@ cudaError_t launch_combine(sekv_handle* h, int layer, void* out, float* lse, cud
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
                          float* alpha, int32_t* ids, int32_t* count, void* out, float* lse, cudaStream_t s);
 cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s);
-size_t fused_smem_bytes(const sekv_handle* h, FusedParams* P);
-int fused_occupancy(const sekv_handle* h);
+size_t fused_region_bytes(const sekv_handle* h, FusedParams* P);
+int fused_warps(const sekv_handle* h);
+int fused_route_spans(const sekv_handle* h);
 
 inline uint8_t* ws(const sekv_handle* h, int64_t off) { return h->dev + off; }
 
