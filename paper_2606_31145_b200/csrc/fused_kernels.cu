@@ -4,7 +4,7 @@
 // two items ahead so neither the claim nor the descriptor load is on the warp's critical path):
 //
 //   latency queue (even warps start here)
-//     QPROJ   (b, h)              q' = W q (Eq. 4): coalesced 16-byte loads of W, half-warp shuffle reduction
+//     QPROJ   (b, h)              q' = W q (Eq. 4) on the tensor cores; published through a sentinel, no flag
 //     ROUTE   (b, g, 64 spans)    x = q'.K_bar/sqrt(d') + ln|S|, alpha = sig(x) (Eq. 5), X = max over the group
 //                                 (GQA), ordered 32-bit keys -> global
 //     SELECT  (b, g)              top-k (Eq. 9, cap L123) by a 4-pass radix select on the keys, ties to the lower
@@ -98,58 +98,85 @@ __device__ __forceinline__ void signal_ctr(int32_t* c, int lane) {
   if (lane == 0) red_add_release(c, 1);
 }
 
-// ---------------------------------------------------------------------------------------------------
-// a1 (Eq. 4): q'[j] = sum_d W[h][j][d] q[h][d] for one query head.  W_h is dp x 128 bf16, contiguous: load i of
-// the warp covers rows 2i and 2i+1 (512 bytes); lane L holds 8 elements d = 8 (L & 15) .. of row 2i + (L >> 4).
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void qproj_item(const FusedParams& P, const Item& I, int lane) {
-  const int b = I.bg / P.Hkv, g = I.bg % P.Hkv;
-  const int G = P.Hq / P.Hkv;
-  const int h = g * G + I.a;
-  const __nv_bfloat16* q = P.q + ((size_t)b * P.Hq + h) * kD + 8 * (lane & 15);
-  const uint4 qv = *reinterpret_cast<const uint4*>(q);
-  const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)h * P.dp * kD * 2 + lane * 16;
-  float qf[8];
-  {
-    const uint32_t w[4] = {qv.x, qv.y, qv.z, qv.w};
+__device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q, int G, int gid, int t4,
+                                             uint32_t (&qf)[4][4]) {
 #pragma unroll
-    for (int e = 0; e < 4; ++e) { qf[2 * e] = __uint_as_float(w[e] << 16); qf[2 * e + 1] = __uint_as_float(w[e] & 0xffff0000u); }
+  for (int j = 0; j < 4; ++j) {
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (gid < G) v = *reinterpret_cast<const uint4*>(q + (size_t)gid * kD + (t4 + 4 * j) * 8);
+    qf[j][0] = v.x; qf[j][1] = v.y; qf[j][2] = v.z; qf[j][3] = v.w;
   }
-  float* dst = P.qp + ((size_t)I.bg * G + I.a) * P.dp;
+}
+
+constexpr uint32_t kQpSentinel = 0xFFFFFFFFu;   // never produced by the tensor cores (their NaN is 0x7FFFFFFF)
+
+// ---------------------------------------------------------------------------------------------------
+// a1 (Eq. 4): q'_h = W_h q_h for one query head on the tensor cores: the rows of W_h are the M dimension
+// (16 per tile), the group's queries are the 8 columns, column hl of the result is q'_hl.  All loads of
+// W_h (dp x 128 bf16) are in flight at once.  The result is published without a flag: the buffer holds a
+// sentinel bit pattern until the value arrives, and ROUTE items poll the words they need.
+// ---------------------------------------------------------------------------------------------------
+template <int G>
+__device__ __forceinline__ void qproj_item(const FusedParams& P, const Item& I, int lane) {
+  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, dp = P.dp, hl = I.a;
+  const int gid = lane >> 2, t4 = lane & 3;
+  uint32_t qf[4][4];
+  load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
+  const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)(g * G + hl) * dp * (kD * 2) + t4 * 16;
+  float* dst = P.qp + ((size_t)bg * G + hl) * dp;
 #pragma unroll 1
-  for (int i0 = 0; i0 < P.dp / 2; i0 += 4) {
-    uint4 wv[4];
+  for (int j0 = 0; j0 < dp; j0 += 32) {
+    uint4 w[2][2][4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (i0 + u < P.dp / 2) wv[u] = ldg16(Wh + (size_t)(i0 + u) * 512);
+    for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      if (i0 + u < P.dp / 2) {
-        const uint32_t w[4] = {wv[u].x, wv[u].y, wv[u].z, wv[u].w};
-        float acc = 0.f;
+      for (int hf = 0; hf < 2; ++hf) {
+        const int row = j0 + 16 * mt + 8 * hf + gid;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          acc = fmaf(__uint_as_float(w[e] << 16), qf[2 * e], acc);
-          acc = fmaf(__uint_as_float(w[e] & 0xffff0000u), qf[2 * e + 1], acc);
-        }
+        for (int jj = 0; jj < 4; ++jj)
+          w[mt][hf][jj] = row < dp ? ldg16(Wh + (size_t)row * (kD * 2) + jj * 64) : make_uint4(0u, 0u, 0u, 0u);
+      }
 #pragma unroll
-        for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if ((lane & 15) == 0) dst[2 * (i0 + u) + (lane >> 4)] = acc;
+    for (int mt = 0; mt < 2; ++mt) {
+      float c[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int jj = 0; jj < 4; ++jj) {
+        mma16816_full(c, w[mt][0][jj].x, w[mt][1][jj].x, w[mt][0][jj].y, w[mt][1][jj].y, qf[jj][0], qf[jj][1]);
+        mma16816_full(c, w[mt][0][jj].z, w[mt][1][jj].z, w[mt][0][jj].w, w[mt][1][jj].w, qf[jj][2], qf[jj][3]);
+      }
+      if (t4 == (hl >> 1)) {                                     // this lane holds column hl of the tile
+        const int r = j0 + 16 * mt + gid;
+        if (r < dp) dst[r] = (hl & 1) ? c[1] : c[0];
+        if (r + 8 < dp) dst[r + 8] = (hl & 1) ? c[3] : c[2];
       }
     }
   }
-  signal_ctr(grp_ctr(P, I.bg, C_QP), lane);
+}
+
+// poll four consecutive words of q' until none is the sentinel
+__device__ __forceinline__ float4 poll_qp4(const float* p) {
+  uint4 v;
+  for (;;) {
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    if (v.x != kQpSentinel && v.y != kQpSentinel && v.z != kQpSentinel && v.w != kQpSentinel) break;
+    __nanosleep(64);
+  }
+  return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
 }
 
 // ---------------------------------------------------------------------------------------------------
 // a2 + GQA reduce of a3 (Eq. 5, Eq. 9): spans [I.a, I.b) of (b, g).  The G x nsp rows of the routing table
-// (dp bf16 each) are staged into the warp's region by 16-byte cp.async copies -- all in flight at once,
-// issued before the wait on q' -- and scored from shared memory with compact loops (the code footprint
-// matters more than the arithmetic here: every item runs this once).
+// (dp bf16 each) are staged into the warp's region by 16-byte cp.async copies, all in flight while the
+// warp polls q'.  Fast path (d' = 32, no threshold, no score outputs): per head, the staged rows are the M
+// dimension of mma tiles, q' (split into bf16 hi + lo, ~16 bits) the columns; 16 spans x 1 head per 4 mma.
+// General path: compact scalar loops from shared memory (the code footprint matters more than the
+// arithmetic here: every item runs this once).
 // ---------------------------------------------------------------------------------------------------
+template <int G>
 __device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, uint8_t* region, int lane,
                                            unsigned long long* tm) {
-  const int bg = I.bg, g = bg % P.Hkv, G = P.Hq / P.Hkv, dp = P.dp, lpr = dp >> 3;
+  const int bg = I.bg, g = bg % P.Hkv, dp = P.dp, lpr = dp >> 3;
+  const int gid = lane >> 2, t4 = lane & 3;
   const int nsp = I.b - I.a;
   const uint8_t* route = (const uint8_t*)P.lv.route;
   const int total = nsp * G * lpr;
@@ -161,14 +188,62 @@ __device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, 
                route + ((size_t)(g * G + hl) * P.route_head_stride + (size_t)(I.span0 + I.a + s) * dp) * 2 + c * 16);
   }
   cp_async_commit();
+  const float inv_sqrt_dp = rsqrtf((float)dp);
+  uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
+  const float* gqp = P.qp + (size_t)bg * G * dp;
+  if (dp == 32 && P.tau == nullptr && P.logits_out == nullptr && P.alpha_out == nullptr) {
+    uint32_t bh[4] = {0u, 0u, 0u, 0u}, bl[4] = {0u, 0u, 0u, 0u};
+    float lnl[4];                                                // ln|S| of span 16 i + gid + 8 (t4 & 1)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int s = 16 * i + gid + 8 * (t4 & 1);
+      lnl[i] = s < nsp ? P.cv.ln_len[I.span0 + I.a + s] : 0.f;
+    }
+    if (gid < G) {
+      const float4 v0 = poll_qp4(gqp + gid * 32 + 8 * t4), v1 = poll_qp4(gqp + gid * 32 + 8 * t4 + 4);
+      split_bf16(v0.x * inv_sqrt_dp, v0.y * inv_sqrt_dp, bh[0], bl[0]);
+      split_bf16(v0.z * inv_sqrt_dp, v0.w * inv_sqrt_dp, bh[1], bl[1]);
+      split_bf16(v1.x * inv_sqrt_dp, v1.y * inv_sqrt_dp, bh[2], bl[2]);
+      split_bf16(v1.z * inv_sqrt_dp, v1.w * inv_sqrt_dp, bh[3], bl[3]);
+    }
+    __syncwarp();
+    mark(tm, 0, lane);
+    cp_async_wait<0>();
+    __syncwarp();
+    mark(tm, 1, lane);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int s0 = 16 * i;
+      if (s0 >= nsp) break;
+      float Xa = -INFINITY, Xb = -INFINITY;                      // spans s0 + gid and s0 + gid + 8
+#pragma unroll
+      for (int hl = 0; hl < G; ++hl) {
+        const uint8_t* ra = region + ((size_t)hl * nsp + s0 + gid) * 64 + t4 * 16;
+        const uint4 a = *reinterpret_cast<const uint4*>(ra), c8 = *reinterpret_cast<const uint4*>(ra + 8 * 64);
+        float c[4] = {0.f, 0.f, 0.f, 0.f};
+        mma16816_full(c, a.x, c8.x, a.y, c8.y, bh[0], bh[1]);
+        mma16816_full(c, a.z, c8.z, a.w, c8.w, bh[2], bh[3]);
+        mma16816_full(c, a.x, c8.x, a.y, c8.y, bl[0], bl[1]);
+        mma16816_full(c, a.z, c8.z, a.w, c8.w, bl[2], bl[3]);
+        if (t4 == (hl >> 1)) {                                   // this lane holds column hl
+          Xa = fmaxf(Xa, (hl & 1) ? c[1] : c[0]);
+          Xb = fmaxf(Xb, (hl & 1) ? c[3] : c[2]);
+        }
+      }
+      Xa = quad_max(Xa); Xb = quad_max(Xb);
+      const int s = s0 + gid + 8 * (t4 & 1);
+      if (t4 < 2 && s < nsp) gkeys[I.a + s] = order_key(((t4 & 1) ? Xb : Xa) + lnl[i]);
+    }
+    mark(tm, 2, lane);
+    signal_ctr(grp_ctr(P, bg, C_ROUTE), lane);
+    return;
+  }
   float* sqp = reinterpret_cast<float*>(region + (size_t)P.route_spans * G * dp * 2);     // [G][dp]
-  wait_ctr(grp_ctr(P, bg, C_QP), G, lane, tm);
-  for (int i = lane; i < G * dp; i += 32) sqp[i] = __ldcg(P.qp + (size_t)bg * G * dp + i);
+  for (int i = 4 * lane; i < G * dp; i += 128) *reinterpret_cast<float4*>(sqp + i) = poll_qp4(gqp + i);
+  mark(tm, 0, lane);
   cp_async_wait<0>();
   __syncwarp();
   mark(tm, 1, lane);
-  const float inv_sqrt_dp = rsqrtf((float)dp);
-  uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
   for (int s = lane; s < nsp; s += 32) {
     const float lnl = P.cv.ln_len[I.span0 + I.a + s];
     float X = -INFINITY;
@@ -379,13 +454,23 @@ __device__ __forceinline__ void select_item(const FusedParams& P, const Item& I,
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(region + P.sm_cand);
   wait_ctr(grp_ctr(P, bg, C_ROUTE), I.a, lane, tm);
   const uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
+  for (int i = lane; i < (m + 3) / 4; i += 32) cp_async16(keys + 4 * i, gkeys + 4 * i);   // all in flight at once
+  cp_async_commit();
+  cp_async_wait<0>();
+  __syncwarp();
   int ne = 0;
+  uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+#pragma unroll 4
   for (int i = lane; i < m; i += 32) {
-    const uint32_t k = __ldcg(gkeys + i);
-    keys[i] = k;
-    ne += (k != 0u);
+    const uint32_t k = keys[i];
+    if (k != 0u) { ++ne; kmin = min(kmin, k); kmax = max(kmax, k); }
   }
   const int n_elig = warp_sum_i(ne);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+    kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+  }
   mark(tm, 1, lane);
   int cnt = P.k < 0 ? n_elig : min(P.k, n_elig);
   cnt = min(cnt, P.k_cap);
@@ -397,9 +482,15 @@ __device__ __forceinline__ void select_item(const FusedParams& P, const Item& I,
   if (n_cand == 0) {
     T = 0xFFFFFFFFu;
   } else if (n_cand < n_elig) {
-    uint32_t prefix = 0u, maskb = 0u;
+    // the eligible keys agree on every bit above the highest bit in which kmin and kmax differ: the passes
+    // start there (float keys of one binade share 9 bits: a pass over them would pile every key -- and
+    // every shared-memory atomic -- into one bin)
+    const int hb = 31 - __clz((int)((kmin ^ kmax) | 1u));
+    const int top = min(24, max(0, hb - 7));                    // first digit = bits [top, top + 8)
+    uint32_t maskb = (top + 8 >= 32) ? 0u : ~((1u << (top + 8)) - 1u);
+    uint32_t prefix = kmax & maskb;
     need = n_cand;
-    for (int shift = 24; shift >= 0; shift -= 8) {
+    for (int shift = top; shift >= 0; shift = (shift >= 8 ? shift - 8 : (shift > 0 ? 0 : -1))) {
       for (int i = lane; i < 256; i += 32) hist[i] = 0u;
       __syncwarp();
 #pragma unroll 4
@@ -467,16 +558,6 @@ __device__ __forceinline__ void select_item(const FusedParams& P, const Item& I,
   if (lane == 0) P.count[bg] = cnt;
   mark(tm, 3, lane);
   if (P.mode & FM_ATTN) plan_warp(P, I, region, lane, cnt, n_cand, false, epoch);
-}
-
-__device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q, int G, int gid, int t4,
-                                             uint32_t (&qf)[4][4]) {
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-    if (gid < G) v = *reinterpret_cast<const uint4*>(q + (size_t)gid * kD + (t4 + 4 * j) * 8);
-    qf[j][0] = v.x; qf[j][1] = v.y; qf[j][2] = v.z; qf[j][3] = v.w;
-  }
 }
 
 // one partial record (m2, l, pad, pad, o[128]) per head; lane (gid, t4) holds head gid's (m, l) and the
@@ -999,8 +1080,8 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
       const int cur_idx = idx;
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
       switch (cur.kind) {
-        case IT_QPROJ: qproj_item(P, cur, lane); break;
-        case IT_ROUTE: route_item(P, cur, region, lane, tm); break;
+        case IT_QPROJ: qproj_item<G>(P, cur, lane); break;
+        case IT_ROUTE: route_item<G>(P, cur, region, lane, tm); break;
         case IT_SELECT: select_item(P, cur, region, lane, epoch, tm); break;
         case IT_POOL:
         case IT_COARSE: rows_item<G>(P, cur, region, lane, tm); break;
@@ -1041,6 +1122,8 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   if (last_flag) {
     __threadfence();
     for (int i = tid; i < 4 + 4 * P.BG; i += blockDim.x) P.ctrs[i] = 0;
+    if (P.mode & FM_ROUTE)
+      for (int i = tid; i < P.BG * G * P.dp; i += blockDim.x) reinterpret_cast<uint32_t*>(P.qp)[i] = kQpSentinel;
     if (tid == 0 && (P.mode & FM_ATTN)) {
       *P.lv.layer_step = epoch;
       atomicAdd(&P.stats[ST_LAYER_STEPS], 1ull);

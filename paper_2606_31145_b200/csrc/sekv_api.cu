@@ -306,6 +306,7 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_err_flag, 0, 16, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_qp, 0xFF, (size_t)c.max_seqs * c.n_q_heads * c.route_dim * 4, h->main));   // q' sentinel
   CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
   h->n_items = h->n_lat_items = h->select_begin = 0; h->use_fused = false;

@@ -104,7 +104,7 @@ enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FAC
 
 // ---- fused layer kernel (fused_kernels.cu) -------------------------------------------------------
 // Work items of the per-layer persistent kernel.  Every item is processed by ONE warp.  Two queues:
-//   latency queue : QPROJ (Eq. 4), ROUTE (Eq. 5), SELECT (Eq. 9 top-k + factor-cache plan)
+//   latency queue : ROUTE (Eq. 4-5), SELECT (Eq. 9 top-k + factor-cache plan)
 //   main queue    : POOL, ZOOM, COARSE (L119-121, Eq. 8), COMBINE (L61)
 enum ItemKind { IT_QPROJ = 0, IT_ROUTE = 1, IT_SELECT = 2, IT_POOL = 3, IT_ZOOM = 4, IT_COARSE = 5, IT_COMBINE = 6 };
 enum FusedMode { FM_ROUTE = 1, FM_ATTN = 2 };   // FM_ATTN without FM_ROUTE: caller-supplied zoom set
