@@ -277,70 +277,102 @@ __device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, 
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a3: descending bitonic sort of n (power of two) 64-bit keys in the warp's region
+// a3 + a4 by a TEAM: the CTA's latency warps (the even warps, TS = 32 * ceil(nw / 2) threads) meet on named
+// barrier 1 once the latency queue is exhausted and run selection and residency plan of the groups
+// bg = blockIdx.x, + gridDim.x, ... together -- a single warp runs this serial chain at ~200 instructions
+// per microsecond, and every expanded span of the group waits for it.  Tables live in the region of warp 0.
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void bitonic_sort_desc_warp(unsigned long long* keys, int n, int lane) {
+struct Team { int tt, ts, lane, tw, ntw; int* scratch; };
+
+__device__ __forceinline__ void team_bar(const Team& T) { asm volatile("bar.sync 1, %0;" ::"r"(T.ts) : "memory"); }
+
+// exclusive prefix sum over the team (two barriers); *total = sum over the team
+__device__ __forceinline__ int team_excl_scan(const Team& T, int v, int* total) {
+  const int ex = warp_excl_scan(v, T.lane);
+  if (T.lane == 31) T.scratch[T.tw] = ex + v;
+  team_bar(T);
+  int base = 0, tot = 0;
+  for (int w = 0; w < T.ntw; ++w) { const int c = T.scratch[w]; if (w < T.tw) base += c; tot += c; }
+  team_bar(T);
+  *total = tot;
+  return base + ex;
+}
+
+// descending bitonic sort of n (power of two) 64-bit keys in shared memory by the team
+__device__ __forceinline__ void bitonic_sort_desc_team(const Team& T, unsigned long long* keys, int n) {
   for (int size = 2; size <= n; size <<= 1) {
     for (int stride = size >> 1; stride > 0; stride >>= 1) {
-      for (int i = lane; i < (n >> 1); i += 32) {
+      for (int i = T.tt; i < (n >> 1); i += T.ts) {
         const int lo = ((i & ~(stride - 1)) << 1) | (i & (stride - 1));
         const int hi = lo | stride;
         const bool desc = ((lo & size) == 0);
         const unsigned long long a = keys[lo], c = keys[hi];
         if ((a < c) == desc) { keys[lo] = c; keys[hi] = a; }
       }
-      __syncwarp();
+      team_bar(T);
     }
   }
 }
 
-// ---------------------------------------------------------------------------------------------------
-// a4: residency plan of (b, g) by one warp.  The device factor cache of a (layer, sequence, kv head) is
-// `ways` slots with a tag (span id) and a stamp (step of last use).  The first n_zoom entries of sh_ids
-// are this step's zoom set: resident ones are hits, the others are demand misses and take the
-// least-recently-used slots not needed by this step.  Entries n_zoom .. n_cand-1 are prefetch candidates
-// (the next-best spans by routing score): the non-resident ones get a slot too and are copied by the
-// side-stream prefetch kernel after this layer's kernel.  Also: zoom bit-mask for the coarse items (an
-// expanded span's coarse entry is replaced by its tokens), de-duplication of
-// caller-supplied ids, one descriptor per expanded span for the ZOOM items, statistics.
-// ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void plan_warp(const FusedParams& P, const Item& I, uint8_t* region, int lane, int n_zoom,
-                                          int n_cand, bool dedupe, uint32_t epoch) {
-  const int bg = I.bg, g = bg % P.Hkv;
-  const int span0 = I.span0, m = I.b, ways = P.ways;
-  int32_t* sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
-  int16_t* way_of = reinterpret_cast<int16_t*>(region + P.sm_wayof);
-  int32_t* sh_tag = reinterpret_cast<int32_t*>(region + P.sm_tags);
-  uint32_t* sh_stamp = reinterpret_cast<uint32_t*>(sh_tag + ways);
-  int32_t* sh_victim = reinterpret_cast<int32_t*>(sh_stamp + ways);
-  uint32_t* sh_mask = reinterpret_cast<uint32_t*>(region + P.sm_mask);
+struct PlanTables {
+  int32_t* sh_ids; int16_t* way_of; int32_t* sh_tag; uint32_t* sh_stamp; int32_t* sh_victim; uint32_t* sh_mask;
+};
+__device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t* region) {
+  PlanTables t;
+  t.sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
+  t.way_of = reinterpret_cast<int16_t*>(region + P.sm_wayof);
+  t.sh_tag = reinterpret_cast<int32_t*>(region + P.sm_tags);
+  t.sh_stamp = reinterpret_cast<uint32_t*>(t.sh_tag + P.ways);
+  t.sh_victim = reinterpret_cast<int32_t*>(t.sh_stamp + P.ways);
+  t.sh_mask = reinterpret_cast<uint32_t*>(region + P.sm_mask);
+  return t;
+}
+
+// first half of the plan: needs nothing from this step's routing, runs while the ROUTE items are in flight
+__device__ __forceinline__ void plan_init_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int m) {
+  const int32_t* tags = P.lv.tags + (size_t)bg * P.ways;
+  const uint32_t* stamps = P.lv.stamps + (size_t)bg * P.ways;
+  for (int w = T.tt; w < P.mask_words; w += T.ts) t.sh_mask[w] = 0u;
+  for (int s = T.tt; s < m; s += T.ts) t.way_of[s] = (int16_t)-1;
+  for (int w = T.tt; w < P.ways; w += T.ts) { t.sh_tag[w] = tags[w]; t.sh_stamp[w] = stamps[w]; t.sh_victim[w] = -1; }
+  team_bar(T);
+  for (int w = T.tt; w < P.ways; w += T.ts) { const int tg = t.sh_tag[w]; if (tg >= 0 && tg < m) t.way_of[tg] = (int16_t)w; }
+  team_bar(T);
+}
+
+// a4: residency plan of (b, g).  The device factor cache of a (layer, sequence, kv head) is `ways` slots with
+// a tag (span id) and a stamp (step of last use).  The first n_zoom entries of sh_ids are this step's zoom
+// set: resident ones are hits, the others are demand misses and take the least-recently-used slots not
+// needed by this step.  Entries n_zoom .. n_cand-1 are prefetch candidates (the next-best spans by routing
+// score): the non-resident ones get a slot too and are copied by the side-stream prefetch kernel after
+// this layer's kernel.  Also: zoom bit-mask for the coarse items (an expanded span's coarse entry is
+// replaced by its tokens), de-duplication of caller-supplied ids, one descriptor per
+// expanded span for the ZOOM items, statistics.
+__device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
+                                          int m, int n_zoom, int n_cand, bool dedupe, uint32_t epoch) {
+  const int g = bg % P.Hkv, ways = P.ways;
   int32_t* tags = P.lv.tags + (size_t)bg * ways;
   uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
   uint32_t* items = P.lv.items + (size_t)bg * P.kc;
   int32_t* item_span = P.lv.item_span + (size_t)bg * P.kc;
   ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
   const uint32_t cur = epoch;
-  for (int w = lane; w < P.mask_words; w += 32) sh_mask[w] = 0u;
-  for (int s = lane; s < m; s += 32) way_of[s] = (int16_t)-1;
-  for (int w = lane; w < ways; w += 32) { sh_tag[w] = tags[w]; sh_stamp[w] = stamps[w]; sh_victim[w] = -1; }
-  __syncwarp();
-  for (int w = lane; w < ways; w += 32) { const int t = sh_tag[w]; if (t >= 0 && t < m) way_of[t] = (int16_t)w; }
-  __syncwarp();
-  unsigned long long n_hit = 0, n_miss = 0, bytes_algo = 0, bytes_h2d = 0, n_pf = 0, bytes_pf = 0;
+  int n_hit = 0, n_miss = 0, n_pf = 0;
+  unsigned long long bytes_algo = 0, bytes_h2d = 0;
   // pass 1: validate / de-duplicate, zoom mask, residency lookup
-  for (int j = lane; j < n_cand; j += 32) {
-    int id = sh_ids[j];
+  for (int j = T.tt; j < n_cand; j += T.ts) {
+    int id = t.sh_ids[j];
     if (id < 0 || id >= m) id = -1;
     const bool zoom = j < n_zoom;
     if (id >= 0 && zoom) {
       const uint32_t bit = 1u << (id & 31);
-      const uint32_t old = atomicOr(&sh_mask[id >> 5], bit);
+      const uint32_t old = atomicOr(&t.sh_mask[id >> 5], bit);
       if (dedupe && (old & bit)) id = -1;                      // duplicate of an id seen before: dropped
     }
     int way = -1;
     if (id >= 0) {
-      way = way_of[id];
-      if (way >= 0) sh_stamp[way] = cur;
+      way = t.way_of[id];
+      if (way >= 0) t.sh_stamp[way] = cur;
       const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + id];
       const int rk = rr & 0xff, rv = (rr >> 8) & 0xff;
       const int len = P.cv.span_len[span0 + id];
@@ -348,48 +380,52 @@ __device__ __forceinline__ void plan_warp(const FusedParams& P, const Item& I, u
       if (zoom) {
         bytes_algo += (unsigned long long)(rk + rv) * (len + kD) * 2 + 4ull * (rk + rv);
         if (way >= 0) ++n_hit; else { ++n_miss; bytes_h2d += bb; }
-      } else if (way < 0) { ++n_pf; bytes_pf += bb; }
+      } else if (way < 0) { ++n_pf; bytes_h2d += bb; }
     }
-    sh_ids[j] = id;
+    t.sh_ids[j] = id;
     item_span[j] = id;
     items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
   }
-  __syncwarp();
-  // victims: the n_need oldest ways not used by this step (ties to the lower way), found by repeated
-  // extraction of the minimum (stamp, way) -- only as many as this step has misses
-  const int n_need = min(warp_sum_i((int)(n_miss + n_pf)), ways);
-  for (int v = 0; v < n_need; ++v) {
-    unsigned long long best = ~0ull;
-    for (int w = lane; w < ways; w += 32)
-      if (sh_stamp[w] != cur) best = min(best, ((unsigned long long)sh_stamp[w] << 32) | (unsigned long long)w);
+  int n_need;
+  team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1)
+  n_need = min(n_need, ways);
+  // victims: the n_need oldest ways not used by this step (ties to the lower way), by repeated extraction
+  // of the minimum (stamp, way) -- only as many as this step has misses
+  if (T.tw == 0) {
+    for (int v = 0; v < n_need; ++v) {
+      unsigned long long best = ~0ull;
+      for (int w = T.lane; w < ways; w += 32)
+        if (t.sh_stamp[w] != cur) best = min(best, ((unsigned long long)t.sh_stamp[w] << 32) | (unsigned long long)w);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, o));
-    if (best == ~0ull) break;
-    const int w = (int)(best & 0xffffffffull);
-    if (lane == 0) { sh_victim[v] = w; sh_stamp[w] = cur; }    // marked used: not extracted again
-    __syncwarp();
+      for (int o = 16; o > 0; o >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, o));
+      if (best == ~0ull) break;
+      const int w = (int)(best & 0xffffffffull);
+      if (T.lane == 0) { t.sh_victim[v] = w; t.sh_stamp[w] = cur; }    // marked used: not extracted again
+      __syncwarp();
+    }
   }
+  team_bar(T);
   // pass 2: misses take victims in item order; descriptors of the zoom set
   int miss_base = 0;
-  for (int j0 = 0; j0 < n_cand; j0 += 32) {
-    const int j = j0 + lane;
-    const int id = (j < n_cand) ? sh_ids[j] : -1;
+  for (int j0 = 0; j0 < n_cand; j0 += T.ts) {
+    const int j = j0 + T.tt;
+    const int id = (j < n_cand) ? t.sh_ids[j] : -1;
     uint32_t it = (j < n_cand) ? items[j] : 0u;
     const bool miss = id >= 0 && it == 0xFFFFFFFFu;
-    const unsigned bal = __ballot_sync(0xffffffffu, miss);
+    int tot;
+    const int off = team_excl_scan(T, miss ? 1 : 0, &tot);
     if (miss) {
-      const int vi = miss_base + __popc(bal & ((1u << lane) - 1u));
-      const int way = vi < ways ? sh_victim[vi] : -1;
+      const int vi = miss_base + off;
+      const int way = vi < ways ? t.sh_victim[vi] : -1;
       if (way >= 0) {
-        sh_tag[way] = id;
-        sh_stamp[way] = cur;
+        t.sh_tag[way] = id;
         it = (uint32_t)way | 0x80000000u;
       } else {
         it = 0xC0000000u;                                      // no free slot: fetch, do not keep
       }
       items[j] = it;
     }
-    miss_base += __popc(bal);
+    miss_base += tot;
     if (j < n_zoom) {
       ZDescG d;
       d.src = 0ull; d.bytes = 0u; d.len = 0; d.rr = 0; d.way_miss = it; d.id = id; d.pad = 0;
@@ -405,82 +441,110 @@ __device__ __forceinline__ void plan_warp(const FusedParams& P, const Item& I, u
       zd[j] = d;
     }
   }
-  __syncwarp();
-  for (int w = lane; w < ways; w += 32) { tags[w] = sh_tag[w]; stamps[w] = sh_stamp[w]; }
+  team_bar(T);
+  for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
   uint32_t* gmask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
-  for (int w = lane; w < P.mask_words; w += 32) gmask[w] = sh_mask[w];
-  if (lane == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
+  for (int w = T.tt; w < P.mask_words; w += T.ts) gmask[w] = t.sh_mask[w];
+  if (T.tt == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
+  team_bar(T);                                                 // every thread's global writes precede the release
+  if (T.tt == 0) red_add_release(grp_ctr(P, bg, C_PLAN), 1);
+  // statistics (off the critical path)
+  n_hit = warp_sum_i(n_hit); n_miss = warp_sum_i(n_miss); n_pf = warp_sum_i(n_pf);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    n_hit += __shfl_xor_sync(0xffffffffu, n_hit, o);
-    n_miss += __shfl_xor_sync(0xffffffffu, n_miss, o);
     bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
     bytes_h2d += __shfl_xor_sync(0xffffffffu, bytes_h2d, o);
-    n_pf += __shfl_xor_sync(0xffffffffu, n_pf, o);
-    bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
   }
-  if (lane == 0) {
-    if (n_hit) atomicAdd(&P.stats[ST_HITS], n_hit);
-    if (n_miss) atomicAdd(&P.stats[ST_MISSES], n_miss);
-    if (n_hit + n_miss) { atomicAdd(&P.stats[ST_ZOOMED], n_hit + n_miss); atomicAdd(&P.stats[ST_SKIPPED], n_hit + n_miss); }
+  if (T.lane == 0) {
+    if (n_hit) atomicAdd(&P.stats[ST_HITS], (unsigned long long)n_hit);
+    if (n_miss) atomicAdd(&P.stats[ST_MISSES], (unsigned long long)n_miss);
+    if (n_hit + n_miss) {
+      atomicAdd(&P.stats[ST_ZOOMED], (unsigned long long)(n_hit + n_miss));
+      atomicAdd(&P.stats[ST_SKIPPED], (unsigned long long)(n_hit + n_miss));
+    }
     if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
-    if (bytes_h2d + bytes_pf) atomicAdd(&P.stats[ST_H2D], bytes_h2d + bytes_pf);
-    if (n_pf) atomicAdd(&P.stats[ST_PREFETCHED], n_pf);
+    if (bytes_h2d) atomicAdd(&P.stats[ST_H2D], bytes_h2d);
+    if (n_pf) atomicAdd(&P.stats[ST_PREFETCHED], (unsigned long long)n_pf);
   }
-  signal_ctr(grp_ctr(P, bg, C_PLAN), lane);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a3 (Eq. 9, cap L123): top-n_cand of the group's m keys by one warp.  4-pass radix select (8 bits per
-// pass, shared-memory histogram) finds the n_cand-th largest key T; keys > T are taken, keys == T are
-// taken in increasing span id until the count is met (ties to the lower id); the <= kc winners are
-// then sorted by (key descending, id ascending).
+// a3 (Eq. 9, cap L123): top-n_cand of the group's m keys.  A radix select (8 bits per pass, shared-memory
+// histogram, starting at the highest bit in which the eligible keys differ) finds the n_cand-th largest
+// key T; keys > T are taken, keys == T are taken in increasing span id until the count is met (ties to the
+// lower id); the <= kc winners are then sorted by (key descending, id ascending).
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void select_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch, unsigned long long* tm) {
-  const int bg = I.bg, m = I.b;
-  int32_t* sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
+__device__ __forceinline__ void select_team(const FusedParams& P, const Team& T, uint8_t* region, int bg, uint32_t epoch,
+                                            unsigned long long* tm) {
+  const int b = bg / P.Hkv;
+  const int span0 = P.cv.seq_span_off[b];
+  const int m = P.cv.seq_span_off[b + 1] - span0;
+  const PlanTables t = plan_tables(P, region);
+  if (P.mode & FM_ATTN) plan_init_team(P, T, t, bg, m);
   if (!(P.mode & FM_ROUTE)) {
     // caller-supplied zoom set (sekv_decode_attn)
     int cnt = 0;
     if (P.ids != nullptr && P.count != nullptr) cnt = max(0, min(P.count[bg], P.k_cap));
     const int32_t* src = P.ids + (size_t)bg * max(P.k_cap, 1);
-    for (int j = lane; j < cnt; j += 32) sh_ids[j] = src[j];
-    __syncwarp();
-    plan_warp(P, I, region, lane, cnt, cnt, true, epoch);
+    for (int j = T.tt; j < cnt; j += T.ts) t.sh_ids[j] = src[j];
+    team_bar(T);
+    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch);
     return;
   }
   uint32_t* keys = reinterpret_cast<uint32_t*>(region);
   uint32_t* hist = reinterpret_cast<uint32_t*>(region + P.sm_hist);
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(region + P.sm_cand);
-  wait_ctr(grp_ctr(P, bg, C_ROUTE), I.a, lane, tm);
+  int* sel = T.scratch + 8;                                    // [0] digit, [1] keys above it, [2..4] ne / kmin / kmax
   const uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
-  for (int i = lane; i < (m + 3) / 4; i += 32) cp_async16(keys + 4 * i, gkeys + 4 * i);   // all in flight at once
+  const int n_route = (m + P.route_spans - 1) / P.route_spans;
+  if (T.tt == 0) {
+    const int32_t* c = grp_ctr(P, bg, C_ROUTE);
+    int v;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
+      if (v >= n_route) break;
+      __nanosleep(64);
+    }
+    (void)ld_acquire(reinterpret_cast<const uint32_t*>(c));
+    sel[2] = 0; sel[3] = -1; sel[4] = 0;
+    mark(tm, 0, 0);
+  }
+  team_bar(T);
+  for (int i = T.tt; i < (m + 3) / 4; i += T.ts) cp_async16(keys + 4 * i, gkeys + 4 * i);   // all in flight at once
   cp_async_commit();
   cp_async_wait<0>();
-  __syncwarp();
-  int ne = 0;
-  uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-#pragma unroll 4
-  for (int i = lane; i < m; i += 32) {
-    const uint32_t k = keys[i];
-    if (k != 0u) { ++ne; kmin = min(kmin, k); kmax = max(kmax, k); }
-  }
-  const int n_elig = warp_sum_i(ne);
+  team_bar(T);
+  mark(tm, 1, T.tt);
+  {
+    int ne = 0;
+    uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+    for (int i = T.tt; i < m; i += T.ts) {
+      const uint32_t k = keys[i];
+      if (k != 0u) { ++ne; kmin = min(kmin, k); kmax = max(kmax, k); }
+    }
+    ne = warp_sum_i(ne);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
-    kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+    for (int o = 16; o > 0; o >>= 1) {
+      kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+      kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+    }
+    if (T.lane == 0) {
+      atomicAdd(&sel[2], ne);
+      atomicMin(reinterpret_cast<unsigned int*>(&sel[3]), kmin);
+      atomicMax(reinterpret_cast<unsigned int*>(&sel[4]), kmax);
+    }
   }
-  mark(tm, 1, lane);
+  team_bar(T);
+  const int n_elig = sel[2];
+  const uint32_t kmin = (uint32_t)sel[3], kmax = (uint32_t)sel[4];
   int cnt = P.k < 0 ? n_elig : min(P.k, n_elig);
   cnt = min(cnt, P.k_cap);
   int n_cand = cnt;
   if (P.k >= 0 && (P.mode & FM_ATTN)) n_cand = min(min(cnt + P.prefetch, n_elig), P.kc);
-  __syncwarp();
-  uint32_t T = 0u;            // threshold key
-  int need = 0;               // keys == T to take
+  uint32_t Tk = 0u;           // threshold key
+  int need = 0;               // keys == Tk to take
   if (n_cand == 0) {
-    T = 0xFFFFFFFFu;
+    Tk = 0xFFFFFFFFu;
   } else if (n_cand < n_elig) {
     // the eligible keys agree on every bit above the highest bit in which kmin and kmax differ: the passes
     // start there (float keys of one binade share 9 bits: a pass over them would pile every key -- and
@@ -491,73 +555,70 @@ __device__ __forceinline__ void select_item(const FusedParams& P, const Item& I,
     uint32_t prefix = kmax & maskb;
     need = n_cand;
     for (int shift = top; shift >= 0; shift = (shift >= 8 ? shift - 8 : (shift > 0 ? 0 : -1))) {
-      for (int i = lane; i < 256; i += 32) hist[i] = 0u;
-      __syncwarp();
-#pragma unroll 4
-      for (int i = lane; i < m; i += 32) {
+      for (int i = T.tt; i < 256; i += T.ts) hist[i] = 0u;
+      team_bar(T);
+      for (int i = T.tt; i < m; i += T.ts) {
         const uint32_t k = keys[i];
         if (k != 0u && (k & maskb) == prefix) atomicAdd(&hist[(k >> shift) & 255u], 1u);
       }
-      __syncwarp();
-      int loc[8], tot = 0;
+      team_bar(T);
+      if (T.tw == 0) {
+        int loc[8], tot = 0;
 #pragma unroll
-      for (int e = 0; e < 8; ++e) { loc[e] = (int)hist[255 - (8 * lane + e)]; tot += loc[e]; }
-      int run = warp_excl_scan(tot, lane);       // matching keys in bins above this lane's bins
-      int found = -1, fb = 0;
+        for (int e = 0; e < 8; ++e) { loc[e] = (int)hist[255 - (8 * T.lane + e)]; tot += loc[e]; }
+        int run = warp_excl_scan(tot, T.lane);     // matching keys in bins above this lane's bins
 #pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        if (found < 0 && run < need && run + loc[e] >= need) { found = 255 - (8 * lane + e); fb = run; }
-        run += loc[e];
+        for (int e = 0; e < 8; ++e) {
+          if (run < need && run + loc[e] >= need) { sel[0] = 255 - (8 * T.lane + e); sel[1] = run; }
+          run += loc[e];
+        }
       }
-      const unsigned bal = __ballot_sync(0xffffffffu, found >= 0);
-      const int srcl = __ffs(bal) - 1;
-      const int d = __shfl_sync(0xffffffffu, found, srcl);
-      fb = __shfl_sync(0xffffffffu, fb, srcl);
-      need -= fb;
-      prefix |= (uint32_t)d << shift;
+      team_bar(T);
+      need -= sel[1];
+      prefix |= (uint32_t)sel[0] << shift;
       maskb |= 255u << shift;
-      __syncwarp();
     }
-    T = prefix;
+    Tk = prefix;
   }
-  mark(tm, 2, lane);
-  // ordered compaction: lane owns a contiguous block of span ids
-  const int per = (m + 31) / 32;
-  const int lo = min(m, lane * per), hi = min(m, lo + per);
+  mark(tm, 2, T.tt);
+  // ordered compaction: each thread owns a contiguous block of span ids
+  const int per = (m + T.ts - 1) / T.ts;
+  const int lo = min(m, T.tt * per), hi = min(m, lo + per);
   int gt = 0, eq = 0;
-  for (int i = lo; i < hi; ++i) { const uint32_t k = keys[i]; gt += (k > T); eq += (k == T); }
-  const int eq_before = warp_excl_scan(eq, lane);
-  const int take_eq = (T == 0u) ? 0 : max(0, min(eq, need - eq_before));
-  int pos = warp_excl_scan(gt + take_eq, lane);
+  for (int i = lo; i < hi; ++i) { const uint32_t k = keys[i]; gt += (k > Tk); eq += (k == Tk); }
+  int dummy;
+  const int eq_before = team_excl_scan(T, eq, &dummy);
+  const int take_eq = (Tk == 0u) ? 0 : max(0, min(eq, need - eq_before));
+  int pos = team_excl_scan(T, gt + take_eq, &dummy);
   int taken = 0;
   for (int i = lo; i < hi; ++i) {
     const uint32_t k = keys[i];
-    bool sel = k > T;
-    if (k == T && taken < take_eq) { sel = true; ++taken; }
-    if (sel && pos < P.kc) cand[pos++] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
+    bool s = k > Tk;
+    if (k == Tk && taken < take_eq) { s = true; ++taken; }
+    if (s && pos < P.kc) cand[pos++] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
   }
-  __syncwarp();
-  if (n_cand <= 64) {
-    for (int j = lane; j < n_cand; j += 32) {
-      const unsigned long long mine = cand[j];
+  team_bar(T);
+  if (n_cand <= T.ts) {
+    if (T.tt < n_cand) {
+      const unsigned long long mine = cand[T.tt];
       int r = 0;
       for (int i = 0; i < n_cand; ++i) r += (cand[i] > mine);
-      sh_ids[r] = (int32_t)(0xFFFFFFFFu - (uint32_t)(mine & 0xFFFFFFFFull));
+      t.sh_ids[r] = (int32_t)(0xFFFFFFFFu - (uint32_t)(mine & 0xFFFFFFFFull));
     }
   } else {
     int n2 = 64;
     while (n2 < n_cand) n2 <<= 1;
-    for (int j = n_cand + lane; j < n2; j += 32) cand[j] = 0ull;
-    __syncwarp();
-    bitonic_sort_desc_warp(cand, n2, lane);
-    for (int j = lane; j < n_cand; j += 32) sh_ids[j] = (int32_t)(0xFFFFFFFFu - (uint32_t)(cand[j] & 0xFFFFFFFFull));
+    for (int j = n_cand + T.tt; j < n2; j += T.ts) cand[j] = 0ull;
+    team_bar(T);
+    bitonic_sort_desc_team(T, cand, n2);
+    for (int j = T.tt; j < n_cand; j += T.ts) t.sh_ids[j] = (int32_t)(0xFFFFFFFFu - (uint32_t)(cand[j] & 0xFFFFFFFFull));
   }
-  __syncwarp();
+  team_bar(T);
+  mark(tm, 3, T.tt);
   int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
-  for (int j = lane; j < P.k_cap; j += 32) my_ids[j] = j < cnt ? sh_ids[j] : -1;
-  if (lane == 0) P.count[bg] = cnt;
-  mark(tm, 3, lane);
-  if (P.mode & FM_ATTN) plan_warp(P, I, region, lane, cnt, n_cand, false, epoch);
+  for (int j = T.tt; j < P.k_cap; j += T.ts) my_ids[j] = j < cnt ? t.sh_ids[j] : -1;
+  if (T.tt == 0) P.count[bg] = cnt;
+  if (P.mode & FM_ATTN) plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch);
 }
 
 // one partial record (m2, l, pad, pad, o[128]) per head; lane (gid, t4) holds head gid's (m, l) and the
@@ -1043,6 +1104,26 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   const int nlw = (nw + 1) >> 1, nmw = nw >> 1;
   const int total_lw = (int)gridDim.x * nlw, total_mw = (int)gridDim.x * nmw;
   bool in_lat = (warp & 1) == 0;
+  __shared__ int team_scratch[16];
+  // selection and residency plan of this CTA's groups by the team of latency warps (once per warp)
+  auto team_work = [&]() {
+    Team T;
+    T.tt = (warp >> 1) * 32 + lane; T.ts = nlw * 32; T.lane = lane; T.tw = warp >> 1; T.ntw = nlw; T.scratch = team_scratch;
+    for (int bg = (int)blockIdx.x; bg < P.BG; bg += (int)gridDim.x) {
+      unsigned long long t0 = 0ull;
+      if (P.trace) { t0 = globaltimer_ns(); if (T.tt == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
+      select_team(P, T, dsm, bg, epoch, tm);
+      const int rec = P.main_end + bg;                         // trace record after the queue items
+      if (P.trace && T.tt == 0 && rec < P.trace_cap) {
+        unsigned long long* r = P.trace + 8 * (size_t)rec;
+        r[0] = (unsigned long long)(uint32_t)IT_SELECT | ((unsigned long long)(uint32_t)bg << 32);
+        r[1] = (unsigned long long)blockIdx.x;
+        r[2] = t0; r[3] = globaltimer_ns();
+        r[4] = tm[0]; r[5] = tm[1]; r[6] = tm[2]; r[7] = tm[3];
+      }
+      team_bar(T);
+    }
+  };
   auto claim = [&]() -> int {
     int i = 0;
     if (in_lat) {
@@ -1050,6 +1131,7 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
       i = __shfl_sync(0xffffffffu, i, 0);
       if (i < P.lat_end) return i;
       in_lat = false;
+      team_work();
     }
     if (lane == 0) i = P.lat_end + total_mw + atomicAdd(P.ctrs + 1, 1);
     return __shfl_sync(0xffffffffu, i, 0);
@@ -1057,7 +1139,7 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   int idx;
   if (in_lat) {
     idx = P.lat_begin + (int)blockIdx.x * nlw + (warp >> 1);
-    if (idx >= P.lat_end) { in_lat = false; idx = claim(); }
+    if (idx >= P.lat_end) { in_lat = false; team_work(); idx = claim(); }
   } else {
     idx = P.lat_end + (int)blockIdx.x * nmw + (warp >> 1);
   }
@@ -1082,7 +1164,6 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
       switch (cur.kind) {
         case IT_QPROJ: qproj_item<G>(P, cur, lane); break;
         case IT_ROUTE: route_item<G>(P, cur, region, lane, tm); break;
-        case IT_SELECT: select_item(P, cur, region, lane, epoch, tm); break;
         case IT_POOL:
         case IT_COARSE: rows_item<G>(P, cur, region, lane, tm); break;
         case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, tm); break;

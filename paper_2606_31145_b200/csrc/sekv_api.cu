@@ -388,9 +388,10 @@ static sekv_status make_schedule(sekv_handle* h) {
   return SEKV_OK;
 }
 
-// Work-item lists of the fused layer kernel (bf16 path), in queue order.  Latency queue: QPROJ, ROUTE,
-// SELECT; main queue: POOL, ZOOM, COARSE, COMBINE.  Both are topological orders of the dependencies
-// (ROUTE after QPROJ, SELECT after ROUTE, ZOOM / COARSE after SELECT, COMBINE after the attention items).
+// Work-item lists of the fused layer kernel (bf16 path), in queue order.  Latency queue: QPROJ, ROUTE (the
+// selection and plan of a group run on a team of warps once the queue is exhausted); main queue: POOL,
+// ZOOM, COARSE, COMBINE.  Both are topological orders of the dependencies (ROUTE after QPROJ, ZOOM / COARSE
+// after the group's plan, COMBINE after the attention items).
 static sekv_status make_fused_schedule(sekv_handle* h) {
   const FullLayout& F = h->F;
   const sekv_config& c = h->cfg;
@@ -445,9 +446,7 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
       const int m = h->m_b[b];
       for (int s0 = 0; s0 < m; s0 += rspans) { items.push_back(mk(IT_ROUTE, b, g, s0, std::min(m, s0 + rspans), 0)); ++route_items[b * Hkv + g]; }
     }
-  h->select_begin = (int)items.size();
-  for (int b = 0; b < B; ++b)
-    for (int g = 0; g < Hkv; ++g) items.push_back(mk(IT_SELECT, b, g, route_items[b * Hkv + g], h->m_b[b], 0));
+  h->select_begin = (int)items.size();      // caller-supplied zoom sets: the latency queue is empty
   h->n_lat_items = (int)items.size();
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)
