@@ -70,7 +70,7 @@ __device__ __forceinline__ int warp_excl_scan(int v, int lane) {
 
 // per-group counters inside P.ctrs
 __device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
-enum { C_QP = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };
+enum { C_POOL = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };
 
 // spin (lane 0) until the counter reaches `target`
 // (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
@@ -795,7 +795,11 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
           *reinterpret_cast<float2*>(o + 64 * s + 8 * gid + 2 * w) = make_float2(acc[s][w][c], acc[s][w][2 + c]);
     }
   }
-  signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
+  __syncwarp();
+  if (lane == 0) {
+    if (I.kind == IT_POOL) red_add_release(grp_ctr(P, bg, C_POOL), 1);
+    red_add_release(grp_ctr(P, bg, C_ATTN), 1);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1019,14 +1023,19 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
                                              uint32_t& phase, int lane, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, hl = I.a, np = I.np;
   const int G = P.Hq / P.Hkv;
-  wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);
   const float* src = P.partials + ((size_t)I.pbase + (size_t)hl * np) * kPartStride;
   const int cap = P.region_bytes / (kPartStride * 4);
   const float* rec = reinterpret_cast<const float*>(region);
   float M = -INFINITY, L = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  // two phases: the POOL partials (slots [0, I.b)) are complete long before the expanded spans are; they are
+  // merged while those are still running, so only the ZOOM and COARSE partials remain for the tail
+  const int n_pool = I.b;
+  wait_ctr(grp_ctr(P, bg, C_POOL), n_pool, lane, nullptr);
+  bool second = false;
   for (int p0 = 0; p0 < np; p0 += cap) {
-    const int n = min(cap, np - p0);
+    if (!second && p0 >= n_pool) { wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm); second = true; }
+    const int n = min(cap, (second ? np : n_pool) - p0);
     region_fetch(region, src + (size_t)p0 * kPartStride, (uint32_t)(n * kPartStride * 4), bar, phase, lane);
     float mc = -INFINITY;
     for (int p = lane; p < n; p += 32) mc = fmaxf(mc, rec[p * kPartStride]);
@@ -1052,7 +1061,9 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
       acc.x = fmaf(v.x, w, acc.x); acc.y = fmaf(v.y, w, acc.y); acc.z = fmaf(v.z, w, acc.z); acc.w = fmaf(v.w, w, acc.w);
     }
     M = Mn;
+    if (!second && p0 + n >= n_pool) { p0 = n_pool - cap; }     // next round starts at the first non-POOL partial
   }
+  if (!second) wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);  // (no ZOOM / COARSE partials at all)
   const float inv = L > 0.f ? 1.f / L : 0.f;
   const size_t oi = ((size_t)b * P.Hq + (size_t)g * G + hl) * kD + 4 * lane;
   if (P.out_bf16) {
@@ -1100,15 +1111,19 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   uint32_t phase = 0u;
   unsigned long long* tm = P.trace ? &tmid_s[warp * 4] : nullptr;
 
-  // even warps start on the latency queue, odd warps on the main queue; first item static
-  const int nlw = (nw + 1) >> 1, nmw = nw >> 1;
-  const int total_lw = (int)gridDim.x * nlw, total_mw = (int)gridDim.x * nmw;
-  bool in_lat = (warp & 1) == 0;
+  // Latency items are handed out statically to the first warps of the grid (every warp of a CTA takes one), so
+  // the whole latency queue starts at t = 0; what is left of it (large batches) is claimed by the even warps,
+  // which also form the CTA's selection / plan team.  Everything else is claimed from the main queue.
+  const int nlw = (nw + 1) >> 1;
+  const int total_w = (int)gridDim.x * nw, gw = (int)blockIdx.x * nw + warp;
+  const bool team_member = (warp & 1) == 0;
+  bool in_lat = false;
   __shared__ int team_scratch[16];
   // selection and residency plan of this CTA's groups by the team of latency warps (once per warp)
   auto team_work = [&]() {
     Team T;
     T.tt = (warp >> 1) * 32 + lane; T.ts = nlw * 32; T.lane = lane; T.tw = warp >> 1; T.ntw = nlw; T.scratch = team_scratch;
+    team_bar(T);                                               // warp 0 is done with its region (the tables live there)
     for (int bg = (int)blockIdx.x; bg < P.BG; bg += (int)gridDim.x) {
       unsigned long long t0 = 0ull;
       if (P.trace) { t0 = globaltimer_ns(); if (T.tt == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
@@ -1127,21 +1142,22 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   auto claim = [&]() -> int {
     int i = 0;
     if (in_lat) {
-      if (lane == 0) i = P.lat_begin + total_lw + atomicAdd(P.ctrs, 1);
+      if (lane == 0) i = P.lat_begin + total_w + atomicAdd(P.ctrs, 1);
       i = __shfl_sync(0xffffffffu, i, 0);
       if (i < P.lat_end) return i;
       in_lat = false;
       team_work();
     }
-    if (lane == 0) i = P.lat_end + total_mw + atomicAdd(P.ctrs + 1, 1);
+    if (lane == 0) i = P.lat_end + atomicAdd(P.ctrs + 1, 1);
     return __shfl_sync(0xffffffffu, i, 0);
   };
   int idx;
-  if (in_lat) {
-    idx = P.lat_begin + (int)blockIdx.x * nlw + (warp >> 1);
-    if (idx >= P.lat_end) { in_lat = false; team_work(); idx = claim(); }
+  if (gw < P.lat_end - P.lat_begin) {
+    idx = P.lat_begin + gw;
+    in_lat = team_member;
   } else {
-    idx = P.lat_end + (int)blockIdx.x * nmw + (warp >> 1);
+    if (team_member) team_work();
+    idx = claim();
   }
   if (idx < P.main_end) {
     // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular): the
