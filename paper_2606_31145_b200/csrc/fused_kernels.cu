@@ -314,6 +314,25 @@ __device__ __forceinline__ void bitonic_sort_desc_team(const Team& T, unsigned l
   }
 }
 
+__device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, int bg, int g, int span0, int id, uint32_t it,
+                                            uint32_t epoch) {
+  ZDescG d;
+  d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = it; d.id = id; d.epoch0 = epoch; d.epoch1 = epoch;
+  if (id >= 0) {
+    const int gs = span0 + id;
+    const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + gs];
+    const int len = P.cv.span_len[gs];
+    d.len_rr = ((uint32_t)len << 16) | (uint32_t)(rr & 0xffff);
+    d.bytes = (uint32_t)blob_dims(2, len, rr & 0xff, (rr >> 8) & 0xff).bytes;
+    const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
+                                            : P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
+    d.src = (unsigned long long)src;
+  }
+  uint4* o = reinterpret_cast<uint4*>(zd);
+  o[0] = make_uint4((uint32_t)d.src, (uint32_t)(d.src >> 32), d.bytes, d.epoch0);
+  o[1] = make_uint4(d.len_rr, d.way_miss, (uint32_t)d.id, d.epoch1);
+}
+
 struct PlanTables {
   int32_t* sh_ids; int16_t* way_of; int32_t* sh_tag; uint32_t* sh_stamp; int32_t* sh_victim; uint32_t* sh_mask;
 };
@@ -385,7 +404,11 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
     t.sh_ids[j] = id;
     item_span[j] = id;
     items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
+    // hits (and dropped duplicates) publish their descriptor at once: the ZOOM items poll it and start
+    // while the misses are still being given slots
+    if (zoom && (way >= 0 || id < 0)) write_zdesc(P, zd + j, bg, g, span0, id, (uint32_t)max(way, 0), epoch);
   }
+  for (int j = n_zoom + T.tt; j < min(P.k_cap, m); j += T.ts) write_zdesc(P, zd + j, bg, g, span0, -1, 0u, epoch);
   int n_need;
   team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1)
   n_need = min(n_need, ways);
@@ -426,20 +449,7 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       items[j] = it;
     }
     miss_base += tot;
-    if (j < n_zoom) {
-      ZDescG d;
-      d.src = 0ull; d.bytes = 0u; d.len = 0; d.rr = 0; d.way_miss = it; d.id = id; d.pad = 0;
-      if (id >= 0) {
-        const int gs = span0 + id;
-        d.rr = P.lv.dir_rank[(size_t)g * P.spans_cap + gs];
-        d.len = P.cv.span_len[gs];
-        d.bytes = (uint32_t)blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff).bytes;
-        const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
-                                                : P.lv.slots + ((size_t)bg * ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
-        d.src = (unsigned long long)src;
-      }
-      zd[j] = d;
-    }
+    if (miss && j < n_zoom) write_zdesc(P, zd + j, bg, g, span0, id, it, epoch);
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
@@ -957,11 +967,18 @@ __device__ __forceinline__ void region_fetch(uint8_t* region, const void* src, u
   phase ^= 1u;
 }
 
-__device__ __forceinline__ ZDescG load_zdesc(const ZDescG* p) {
-  const uint4 a = __ldcg(reinterpret_cast<const uint4*>(p)), c = __ldcg(reinterpret_cast<const uint4*>(p) + 1);
+// poll a descriptor until both halves carry this launch's stamp
+__device__ __forceinline__ ZDescG poll_zdesc(const ZDescG* p, uint32_t epoch) {
+  uint4 a, c;
+  for (;;) {
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(c.x), "=r"(c.y), "=r"(c.z), "=r"(c.w) : "l"(reinterpret_cast<const uint4*>(p) + 1) : "memory");
+    if (a.w == epoch && c.w == epoch) break;
+    __nanosleep(64);
+  }
   ZDescG d;
   d.src = (unsigned long long)a.x | ((unsigned long long)a.y << 32);
-  d.bytes = a.z; d.len = (int32_t)a.w; d.rr = (int32_t)c.x; d.way_miss = c.y; d.id = (int32_t)c.z; d.pad = 0;
+  d.bytes = a.z; d.epoch0 = a.w; d.len_rr = c.x; d.way_miss = c.y; d.id = (int32_t)c.z; d.epoch1 = c.w;
   return d;
 }
 
@@ -970,29 +987,24 @@ __device__ __forceinline__ ZDescG load_zdesc(const ZDescG* p) {
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
-                                          uint32_t& phase, int lane, unsigned long long* tm) {
+                                          uint32_t& phase, int lane, uint32_t epoch, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
   uint32_t qf[4][4];
   load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
-  wait_ctr(grp_ctr(P, bg, C_PLAN), 1, lane, tm);
-  const int n_zoom = __ldcg(P.plan_counts + 2 * bg);
-  const int j0 = I.a, j1 = min(I.b, n_zoom);
+  const int j0 = I.a, j1 = I.b;                       // the plan stamps every descriptor of the schedule (id -1 = none)
   float M = -INFINITY, L = 0.f;
   float of[16][4];
 #pragma unroll
   for (int n = 0; n < 16; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
   const ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
-  ZDescG dn;
-  dn.id = -1;
-  if (j0 < j1) dn = load_zdesc(zd + j0);
   for (int j = j0; j < j1; ++j) {
-    const ZDescG d = dn;
-    if (j + 1 < j1) dn = load_zdesc(zd + j + 1);
+    const ZDescG d = poll_zdesc(zd + j, epoch);
+    if (j == j0) mark(tm, 0, lane);
     if (d.id < 0) continue;
     region_fetch(region, (const void*)d.src, d.bytes, bar, phase, lane);
     if (j == j0) mark(tm, 1, lane);
-    const BlobDims bd = blob_dims(2, d.len, d.rr & 0xff, (d.rr >> 8) & 0xff);
+    const BlobDims bd = blob_dims(2, (int)(d.len_rr >> 16), d.len_rr & 0xff, (d.len_rr >> 8) & 0xff);
     const int kst = (max(bd.rkp, bd.rvp) + 15) >> 4;
     if (kst <= 1) zoom_span_warp<G, 1>(region, bd, lane, qf, M, L, of);
     else if (kst == 2) zoom_span_warp<G, 2>(region, bd, lane, qf, M, L, of);
@@ -1182,7 +1194,7 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
         case IT_ROUTE: route_item<G>(P, cur, region, lane, tm); break;
         case IT_POOL:
         case IT_COARSE: rows_item<G>(P, cur, region, lane, tm); break;
-        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, tm); break;
+        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, epoch, tm); break;
         default: combine_item(P, cur, region, bar, phase, lane, tm); break;
       }
       if (P.trace && lane == 0 && cur_idx < P.trace_cap) {
@@ -1331,7 +1343,7 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.partials = (float*)ws(h, h->F.off_partials1);
   P.keys = (uint32_t*)ws(h, h->F.off_keys);
   P.qp = (float*)ws(h, h->F.off_qp);
-  P.zdesc = (ZDescG*)ws(h, h->F.off_zdesc);
+  P.zdesc = (ZDescG*)ws(h, h->F.off_zdesc) + (size_t)layer * c.max_seqs * c.n_kv_heads * (std::max(c.k_cap, 1) + std::max(c.prefetch, 0));
   P.ctrs = (int32_t*)ws(h, h->F.off_ctrs) + (size_t)layer * h->F.ctrs_per_layer;
   P.plan_counts = (int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
   P.stats = (unsigned long long*)ws(h, h->F.off_stats);

@@ -116,7 +116,7 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   F->off_keys = cv.take((size_t)B * Hkv * kpb * 8);
   F->ctrs_per_layer = (int)(4 + 4 * B * Hkv);
   F->off_qp = cv.take((size_t)B * Hq * c.route_dim * 4);
-  F->off_zdesc = cv.take((size_t)B * Hkv * kc * sizeof(ZDescG));
+  F->off_zdesc = cv.take((size_t)NL * B * Hkv * kc * sizeof(ZDescG));
   F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);
   F->off_plan_counts = cv.take((size_t)NL * B * Hkv * 2 * 4);
   F->off_layer_step = cv.take((size_t)NL * 4);
@@ -302,6 +302,8 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + h->lay.cache_tags, 0xFF, regions * c.cache_ways * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + h->lay.cache_stamps, 0, regions * c.cache_ways * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_layer_step, 0, (size_t)c.n_layers * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_zdesc, 0, (size_t)c.n_layers * c.max_seqs * c.n_kv_heads *
+                        (std::max(c.k_cap, 1) + std::max(c.prefetch, 0)) * sizeof(ZDescG), h->main));   // stamps restart
   CK(h, cudaMemsetAsync(h->dev + F.off_stats, 0, ST_COUNT * 8, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_err_flag, 0, 16, h->main));

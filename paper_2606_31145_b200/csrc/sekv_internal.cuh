@@ -125,11 +125,11 @@ struct __align__(16) Item {   // 48 bytes: three 16-byte loads
 struct __align__(16) ZDescG {   // what a ZOOM item needs to know about one expanded span (written by the plan)
   unsigned long long src;       // blob address: cache slot (hit) or device alias of the pinned-host store (miss)
   uint32_t bytes;
-  int32_t len;
-  int32_t rr;                   // rank_k | rank_v << 8
-  uint32_t way_miss;            // way | miss << 31
+  uint32_t epoch0;              // the layer's step stamp: both halves carry it, ZOOM items poll until it matches
+  uint32_t len_rr;              // |S| << 16 | rank_k | rank_v << 8
+  uint32_t way_miss;            // way | miss << 31 | no-slot << 30
   int32_t id;                   // local span id, -1 = dropped duplicate
-  int32_t pad;
+  uint32_t epoch1;
 };
 
 struct FusedParams {
@@ -147,7 +147,7 @@ struct FusedParams {
   float* partials;             // records [pbase + hl * np + part][kPartStride]
   uint32_t* keys;              // [BG][keys_stride] ordered routing keys (0 = not eligible)
   float* qp;                   // [BG][G][dp] projected queries
-  ZDescG* zdesc;               // [BG][kc]
+  ZDescG* zdesc;               // [BG][kc] of this layer
   int32_t* ctrs;               // [0] latency queue, [1] main queue, [2] exited CTAs, [3] pad, then per group:
                                // qp_done, route_done, attn_done, plan_flag
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
