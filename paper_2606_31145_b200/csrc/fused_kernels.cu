@@ -70,7 +70,7 @@ __device__ __forceinline__ int warp_excl_scan(int v, int lane) {
 
 // per-group counters inside P.ctrs
 __device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
-enum { C_POOL = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };
+enum { C_EARLY = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };   // C_EARLY: POOL + COARSE items done
 
 // spin (lane 0) until the counter reaches `target`
 // (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
@@ -314,15 +314,16 @@ __device__ __forceinline__ void bitonic_sort_desc_team(const Team& T, unsigned l
   }
 }
 
+// meta = |S| << 16 | rank_k | rank_v << 8 of the span
 __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, int bg, int g, int span0, int id, uint32_t it,
-                                            uint32_t epoch) {
+                                            uint32_t meta, uint32_t epoch) {
   ZDescG d;
   d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = it; d.id = id; d.epoch0 = epoch; d.epoch1 = epoch;
   if (id >= 0) {
     const int gs = span0 + id;
-    const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + gs];
-    const int len = P.cv.span_len[gs];
-    d.len_rr = ((uint32_t)len << 16) | (uint32_t)(rr & 0xffff);
+    const int rr = (int)(meta & 0xffffu);
+    const int len = (int)(meta >> 16);
+    d.len_rr = meta;
     d.bytes = (uint32_t)blob_dims(2, len, rr & 0xff, (rr >> 8) & 0xff).bytes;
     const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
                                             : P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
@@ -335,6 +336,7 @@ __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, in
 
 struct PlanTables {
   int32_t* sh_ids; int16_t* way_of; int32_t* sh_tag; uint32_t* sh_stamp; int32_t* sh_victim; uint32_t* sh_mask;
+  uint32_t* meta;      // [m] |S| << 16 | rank_k | rank_v << 8 of every span of the group
 };
 __device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t* region) {
   PlanTables t;
@@ -344,11 +346,28 @@ __device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t*
   t.sh_stamp = reinterpret_cast<uint32_t*>(t.sh_tag + P.ways);
   t.sh_victim = reinterpret_cast<int32_t*>(t.sh_stamp + P.ways);
   t.sh_mask = reinterpret_cast<uint32_t*>(region + P.sm_mask);
+  t.meta = reinterpret_cast<uint32_t*>(region + P.sm_meta);
   return t;
 }
 
 // first half of the plan: needs nothing from this step's routing, runs while the ROUTE items are in flight
-__device__ __forceinline__ void plan_init_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int m) {
+__device__ __forceinline__ void plan_init_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
+                                               int m) {
+  const int g = bg % P.Hkv;
+  for (int s0 = 0; s0 < m; s0 += 8 * T.ts) {                   // 16 loads in flight per thread
+    int len[8], rr[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int s = min(s0 + u * T.ts + T.tt, m - 1);
+      len[u] = P.cv.span_len[span0 + s];
+      rr[u] = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + s];
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int s = s0 + u * T.ts + T.tt;
+      if (s < m) t.meta[s] = ((uint32_t)len[u] << 16) | (uint32_t)(rr[u] & 0xffff);
+    }
+  }
   const int32_t* tags = P.lv.tags + (size_t)bg * P.ways;
   const uint32_t* stamps = P.lv.stamps + (size_t)bg * P.ways;
   for (int w = T.tt; w < P.mask_words; w += T.ts) t.sh_mask[w] = 0u;
@@ -389,12 +408,13 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       if (dedupe && (old & bit)) id = -1;                      // duplicate of an id seen before: dropped
     }
     int way = -1;
+    uint32_t meta = 0u;
     if (id >= 0) {
       way = t.way_of[id];
       if (way >= 0) t.sh_stamp[way] = cur;
-      const int rr = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + id];
-      const int rk = rr & 0xff, rv = (rr >> 8) & 0xff;
-      const int len = P.cv.span_len[span0 + id];
+      meta = t.meta[id];
+      const int rk = meta & 0xff, rv = (meta >> 8) & 0xff;
+      const int len = (int)(meta >> 16);
       const unsigned long long bb = blob_dims(2, len, rk, rv).bytes;
       if (zoom) {
         bytes_algo += (unsigned long long)(rk + rv) * (len + kD) * 2 + 4ull * (rk + rv);
@@ -406,9 +426,9 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
     items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
     // hits (and dropped duplicates) publish their descriptor at once: the ZOOM items poll it and start
     // while the misses are still being given slots
-    if (zoom && (way >= 0 || id < 0)) write_zdesc(P, zd + j, bg, g, span0, id, (uint32_t)max(way, 0), epoch);
+    if (zoom && (way >= 0 || id < 0)) write_zdesc(P, zd + j, bg, g, span0, id, (uint32_t)max(way, 0), meta, epoch);
   }
-  for (int j = n_zoom + T.tt; j < min(P.k_cap, m); j += T.ts) write_zdesc(P, zd + j, bg, g, span0, -1, 0u, epoch);
+  for (int j = n_zoom + T.tt; j < min(P.k_cap, m); j += T.ts) write_zdesc(P, zd + j, bg, g, span0, -1, 0u, 0u, epoch);
   int n_need;
   team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1)
   n_need = min(n_need, ways);
@@ -449,7 +469,7 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       items[j] = it;
     }
     miss_base += tot;
-    if (miss && j < n_zoom) write_zdesc(P, zd + j, bg, g, span0, id, it, epoch);
+    if (miss && j < n_zoom) write_zdesc(P, zd + j, bg, g, span0, id, it, t.meta[id], epoch);
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
@@ -490,7 +510,7 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
   const int span0 = P.cv.seq_span_off[b];
   const int m = P.cv.seq_span_off[b + 1] - span0;
   const PlanTables t = plan_tables(P, region);
-  if (P.mode & FM_ATTN) plan_init_team(P, T, t, bg, m);
+  if (P.mode & FM_ATTN) plan_init_team(P, T, t, bg, span0, m);
   if (!(P.mode & FM_ROUTE)) {
     // caller-supplied zoom set (sekv_decode_attn)
     int cnt = 0;
@@ -677,20 +697,15 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
     if (t < ntiles) fill(t);
     cp_async_commit();
   }
-  // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L
+  // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L.  EVERY coarse entry is
+  // included (no dependency on this step's zoom set): the ZOOM item of an expanded span subtracts that span's
+  // coarse term again (the softmax numerator and denominator are sums, "replaced by").
   float bias_reg[2] = {0.f, 0.f};
   if (I.kind == IT_COARSE) {
-    wait_ctr(grp_ctr(P, bg, C_PLAN), 1, lane, tm);
-    const uint32_t* mask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       const int row = row_begin + 32 * u + lane;
-      float bv = -INFINITY;
-      if (row < row_end) {
-        const int s = row - A;
-        bv = (__ldcg(mask + (s >> 5)) & (1u << (s & 31))) ? -INFINITY : P.cv.ln_len[I.span0 + s] * kLog2e;
-      }
-      bias_reg[u] = bv;
+      bias_reg[u] = row < row_end ? P.cv.ln_len[I.span0 + row - A] * kLog2e : -INFINITY;
     }
   }
   uint32_t qf[4][4];
@@ -807,7 +822,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   }
   __syncwarp();
   if (lane == 0) {
-    if (I.kind == IT_POOL) red_add_release(grp_ctr(P, bg, C_POOL), 1);
+    red_add_release(grp_ctr(P, bg, C_EARLY), 1);
     red_add_release(grp_ctr(P, bg, C_ATTN), 1);
   }
 }
@@ -1002,6 +1017,17 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
     const ZDescG d = poll_zdesc(zd + j, epoch);
     if (j == j0) mark(tm, 0, lane);
     if (d.id < 0) continue;
+    // the span's coarse entry (k_bar, v_bar, ln|S|) was counted by a COARSE item: loads for taking it out again
+    const size_t crow = ((size_t)g * P.ent_head_stride + (size_t)(I.row0 + I.A + d.id) * kD) * 2;
+    const uint8_t* kbar = (const uint8_t*)P.lv.ent_k + crow;
+    const uint8_t* vbar = (const uint8_t*)P.lv.ent_v + crow;
+    uint4 kc4[4];
+    uint32_t vb[16];
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) kc4[jj] = gid == 0 ? ldg16(kbar + (t4 + 4 * jj) * 16) : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int nd = 0; nd < 16; ++nd) vb[nd] = __ldg(reinterpret_cast<const uint32_t*>(vbar + (8 * nd + 2 * t4) * 2));
+    const float lnl2 = P.cv.ln_len[I.span0 + d.id] * kLog2e;
     region_fetch(region, (const void*)d.src, d.bytes, bar, phase, lane);
     if (j == j0) mark(tm, 1, lane);
     const BlobDims bd = blob_dims(2, (int)(d.len_rr >> 16), d.len_rr & 0xff, (d.len_rr >> 8) & 0xff);
@@ -1009,6 +1035,26 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
     if (kst <= 1) zoom_span_warp<G, 1>(region, bd, lane, qf, M, L, of);
     else if (kst == 2) zoom_span_warp<G, 2>(region, bd, lane, qf, M, L, of);
     else zoom_span_warp<G, 4>(region, bd, lane, qf, M, L, of);
+    {
+      // minus the coarse entry: logit z = q.k_bar/sqrt(d) + ln|S| exactly as the COARSE item computed it
+      float sacc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int jj = 0; jj < 4; ++jj) {
+        mma16816(sacc, qf[jj][0], qf[jj][1], kc4[jj].x, kc4[jj].y);
+        mma16816(sacc, qf[jj][2], qf[jj][3], kc4[jj].z, kc4[jj].w);
+      }
+      const float zc = __shfl_sync(0xffffffffu, sacc[0], lane & ~3);     // column 0 (the entry) of head gid
+      const float z = fmaf(zc, rsqrtf((float)kD) * kLog2e, lnl2);
+      const float M_new = fmaxf(M, z);
+      const float c_old = exp2f(M - M_new), w = exp2f(z - M_new);
+      M = M_new;
+      L = L * c_old - (t4 == 0 ? w : 0.f);                               // L is summed over the quad at the end
+#pragma unroll
+      for (int nd = 0; nd < 16; ++nd) {
+        of[nd][0] = fmaf(-w, __uint_as_float(vb[nd] << 16), of[nd][0] * c_old);
+        of[nd][1] = fmaf(-w, __uint_as_float(vb[nd] & 0xffff0000u), of[nd][1] * c_old);
+      }
+    }
     if (j == j0) mark(tm, 2, lane);
     if ((d.way_miss & 0xC0000000u) == 0x80000000u) {   // demand miss: the blob came over PCIe; keep it in its slot
       int4* dst = reinterpret_cast<int4*>(P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFFFFFu)) * P.slot_bytes);
@@ -1040,10 +1086,10 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
   const float* rec = reinterpret_cast<const float*>(region);
   float M = -INFINITY, L = 0.f;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  // two phases: the POOL partials (slots [0, I.b)) are complete long before the expanded spans are; they are
-  // merged while those are still running, so only the ZOOM and COARSE partials remain for the tail
+  // two phases: the POOL and COARSE partials (slots [0, I.b)) are complete long before the expanded spans
+  // are; they are merged while those are still running, so only the ZOOM partials remain for the tail
   const int n_pool = I.b;
-  wait_ctr(grp_ctr(P, bg, C_POOL), n_pool, lane, nullptr);
+  wait_ctr(grp_ctr(P, bg, C_EARLY), n_pool, lane, nullptr);
   bool second = false;
   for (int p0 = 0; p0 < np; p0 += cap) {
     if (!second && p0 >= n_pool) { wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm); second = true; }
@@ -1220,6 +1266,16 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
       nidx = nnidx;
     }
   }
+  // an exiting warp has nothing left to claim, and the tail of the kernel is latency-bound: pull the tables
+  // that head the next layer's dependency chain (W, routing summaries) into L2 while HBM is idle
+  if (P.next_W != nullptr) {
+    const size_t w_lines = P.next_W_bytes >> 7, r_lines = P.next_route_head_bytes >> 7;
+    for (size_t i = (size_t)gw * 32 + lane; i < w_lines; i += (size_t)total_w * 32)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_W + (i << 7)));
+    for (int h = 0; h < P.Hq; ++h)
+      for (size_t i = (size_t)gw * 32 + lane; i < r_lines; i += (size_t)total_w * 32)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_route + (size_t)h * P.route_head_stride * 2 + (i << 7)));
+  }
   // last CTA out re-arms the queues and counters and advances the layer's step stamp
   __syncthreads();
   if (tid == 0) {
@@ -1291,6 +1347,7 @@ size_t fused_plan_smem(const sekv_handle* h, FusedParams* P) {
   o = round_up_sz(o, 16); P->sm_wayof = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 8) * 2;
   o = round_up_sz(o, 16); P->sm_tags = (int)o; o += (size_t)c.cache_ways * 12;
   o = round_up_sz(o, 16); P->sm_mask = (int)o; o += (size_t)h->mask_words * 4;
+  o = round_up_sz(o, 16); P->sm_meta = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 4) * 4;
   return o;
 }
 
@@ -1362,6 +1419,13 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.route_spans = fused_route_spans(h);
   // queues: [QPROJ, ROUTE | SELECT | POOL, ZOOM, COARSE, COMBINE]
   P.pool_end = h->pool_end;
+  if ((mode & FM_ROUTE) && (mode & FM_ATTN)) {                  // whole-step launches run the layers in order
+    const LayerView nv = layer_view(h, (layer + 1) % c.n_layers);
+    P.next_W = (const uint8_t*)nv.W;
+    P.next_route = (const uint8_t*)nv.route;
+    P.next_W_bytes = (size_t)c.n_q_heads * c.route_dim * kD * 2;
+    P.next_route_head_bytes = (size_t)h->m_tot * c.route_dim * 2;
+  }
   if (mode == FM_ROUTE) { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_lat_items; }
   else if (mode == FM_ATTN) { P.lat_begin = h->select_begin; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }
   else { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }

@@ -406,7 +406,7 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
   if (nw < 1) return SEKV_OK;                               // blobs too large for shared memory: generic path
   h->fused_warps = nw;
   h->fused_grid = h->num_sms;                               // one resident CTA per SM
-  int rows = c.item_rows > 0 ? c.item_rows : 128;
+  int rows = c.item_rows > 0 ? c.item_rows : 64;
   h->fused_item_rows = rows;
   const int crows = std::min(rows, 64);
   int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 1;
@@ -453,7 +453,12 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)
       for (int r0 = 0; r0 < h->A_b[b]; r0 += rows) attn(IT_POOL, b, g, r0, std::min(h->A_b[b], r0 + rows));
-  h->pool_end = (int)items.size();
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) {
+      const int A = h->A_b[b], R = A + h->m_b[b];
+      for (int r0 = A; r0 < R; r0 += crows) attn(IT_COARSE, b, g, r0, std::min(R, r0 + crows));
+    }
+  h->pool_end = (int)items.size();                    // POOL and COARSE items have no dependencies
   if (c.k_cap > 0)
     for (int b = 0; b < B; ++b)
       for (int g = 0; g < Hkv; ++g) {
@@ -461,14 +466,9 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
         for (int j0 = 0; j0 < kmax; j0 += zs) attn(IT_ZOOM, b, g, j0, std::min(kmax, j0 + zs));
       }
   for (int b = 0; b < B; ++b)
-    for (int g = 0; g < Hkv; ++g) {
-      const int A = h->A_b[b], R = A + h->m_b[b];
-      for (int r0 = A; r0 < R; r0 += crows) attn(IT_COARSE, b, g, r0, std::min(R, r0 + crows));
-    }
-  for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)
       for (int hl = 0; hl < G; ++hl) {
-        Item it = mk(IT_COMBINE, b, g, hl, (h->A_b[b] + rows - 1) / rows, 0);   // b = POOL partials
+        Item it = mk(IT_COMBINE, b, g, hl, (h->A_b[b] + rows - 1) / rows + (h->m_b[b] + crows - 1) / crows, 0);   // b = POOL + COARSE partials
         it.pbase = pbase[b * Hkv + g]; it.np = nparts[b * Hkv + g];
         items.push_back(it);
       }

@@ -153,7 +153,10 @@ struct FusedParams {
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
   unsigned long long* stats;
   const uint8_t* host_arena;   // device alias of the pinned host factor store
-  unsigned long long* trace;   // null, or 4 x u64 per item (sekv_set_trace)
+  unsigned long long* trace;   // null, or 8 x u64 per item (sekv_set_trace)
+  const uint8_t* next_W;       // W and routing table of the layer that runs next: prefetched into L2 by exiting warps
+  const uint8_t* next_route;
+  size_t next_W_bytes, next_route_head_bytes;
   size_t ent_head_stride, route_head_stride;
   int64_t slot_bytes, trace_cap;
   int32_t lat_begin, lat_end, main_end;         // item index ranges of the two queues
@@ -162,7 +165,7 @@ struct FusedParams {
   int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, keys_stride, out_bf16;
   int32_t region_bytes;                          // per-warp shared-memory region
   int32_t route_spans;                           // spans per ROUTE item
-  int32_t sm_cand, sm_ids, sm_wayof, sm_tags, sm_mask, sm_hist;   // byte offsets in the region (select / plan)
+  int32_t sm_cand, sm_ids, sm_wayof, sm_tags, sm_mask, sm_hist, sm_meta;   // byte offsets in the region (select / plan)
 };
 
 // ---- storage-type helpers ------------------------------------------------------------------------
