@@ -680,16 +680,30 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   const float scale2 = rsqrtf((float)kD) * kLog2e;
   const int ntiles = (row_end - row_begin + 15) >> 4;
 
+  // chunk idx = lane + 32 i of a 16 x 256-byte tile is row r = 2 i + (lane >> 4), 16-byte chunk c = lane & 15:
+  // global offsets are contiguous and both swizzles are per-lane constants plus compile-time terms in i
+  const int lr = lane >> 4, lc = lane & 15;
+  const uint32_t dk0 = (uint32_t)(lr * 256 + ((lc ^ (lr << 2)) << 4));
+  const uint32_t dv0 = (uint32_t)(lr * 256);
   auto fill = [&](int t) {
     uint8_t* Ks = region + (t % kStages) * kStageBytes;
     uint8_t* Vs = Ks + 16 * kD * 2;
     const int r0 = row_begin + t * 16;
+    if (r0 + 16 <= row_end) {                                   // full tile: no clamping
+      const size_t src = (size_t)r0 * (kD * 2) + lane * 16;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int idx = lane + 32 * i, r = idx >> 4, c = idx & 15;
-      const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + c * 16;
-      cp_async16(Ks + r * 256 + ((c ^ ((r & 1) << 2)) << 4), Kb + src);
-      cp_async16(Vs + r * 256 + ((c ^ (((r >> 1) & 3) << 1)) << 4), Vb + src);
+      for (int i = 0; i < 8; ++i) {
+        cp_async16(Ks + dk0 + 512 * i, Kb + src + 512 * i);
+        cp_async16(Vs + dv0 + 512 * i + ((lc ^ ((i & 3) << 1)) << 4), Vb + src + 512 * i);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int r = 2 * i + lr;
+        const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + lc * 16;
+        cp_async16(Ks + dk0 + 512 * i, Kb + src);
+        cp_async16(Vs + dv0 + 512 * i + ((lc ^ ((i & 3) << 1)) << 4), Vb + src);
+      }
     }
   };
 #pragma unroll
