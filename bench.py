@@ -7,8 +7,8 @@
 Workload = BASELINE.json configs[2]: Llama-3-8B-shaped, 32 layers, 32 q / 8 kv heads, d_h = 128, bf16,
 batch 4 x 128K context, r = 16, top-k = 32 spans per kv head, SVD factors in a pinned-host store,
 zoomed factors fetched on a side stream into a device factor cache.  A "step" is one decode step of the
-whole hot path over all 32 layers (route -> plan/fetch -> stage 1 -> stage 2 -> combine per layer);
-queries follow an AR(1) stream (rho) so consecutive steps' zoom sets overlap as the cache expects.
+whole hot path over all 32 layers (a1-a7: route, select, plan / fetch, pool + coarse + zoom partials, combine);
+queries follow an AR(1) stream (rho, default 0.99) so consecutive steps' zoom sets overlap as the cache expects.
 Inputs are seeded and synthetic (workloads/).  One JSON line is printed by rank 0.
 """
 from __future__ import annotations
@@ -35,7 +35,10 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--layers", type=int, default=0, help="debug: override the layer count (invalidates the number)")
-    ap.add_argument("--rho", type=float, default=0.9, help="AR(1) coefficient of the query stream")
+    ap.add_argument("--rho", type=float, default=0.99,
+                    help="AR(1) coefficient of the query stream: sets the overlap of consecutive zoom sets, i.e. the "
+                         "factor-cache miss volume (0.99: ~1%% misses, ~29 MB/step over PCIe; 0.9: ~12%%, ~150 MB/step, "
+                         "PCIe-bound; 1.0: no misses).  profiles/ holds the sweep.")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--generic", action="store_true", help="force the generic (non tensor-core) kernels")
@@ -320,7 +323,7 @@ def run_ours(args):
                    "kv_heads": spec.n_kv_heads, "rank": spec.rank, "top_k": spec.top_k, "rho": args.rho,
                    "spans_per_seq": eng.spans_per_seq, "pool_per_seq": eng.pool_per_seq,
                    "cache_ways": cfg.cache_ways, "cache_hit_rate": hit, "graph": not args.no_graph,
-                   "kernels": "generic multi-kernel" if args.generic else "fused persistent layer kernel (mma.sync bf16, TMA bulk factor copies)",
+                   "kernels": "generic multi-kernel" if args.generic else "one persistent kernel per layer-step: warp workers on two dependency-ordered queues (mma.sync bf16, cp.async K/V ring, TMA bulk factor copies)",
                    "prefetch": cfg.prefetch, "stage1_ctas": n_ctas,
                    "l2": "inputs larger than L2: one step streams %.2f GB of tables (L2 = 126 MB), no flush" % (algo_bytes / args.steps / 1e9),
                    "replicas": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",

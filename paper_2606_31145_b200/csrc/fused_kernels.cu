@@ -1172,6 +1172,11 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
   __shared__ int last_flag;
   __shared__ unsigned long long tmid_s[8 * 4];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+  // Programmatic dependent launch: the next layer's grid may be scheduled as soon as this one's CTAs leave
+  // their SMs (its CTAs then sit in the wait below), which hides the launch latency between the dependent
+  // kernels of a step; everything this kernel touches is ordered after the previous grid by the wait.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   uint8_t* region = dsm + (size_t)warp * P.region_bytes;
   uint64_t* bar = &bars[warp];
   const uint32_t epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
@@ -1286,9 +1291,10 @@ __global__ void __launch_bounds__(256, 1) fused_layer_kernel(const __grid_consta
     const size_t w_lines = P.next_W_bytes >> 7, r_lines = P.next_route_head_bytes >> 7;
     for (size_t i = (size_t)gw * 32 + lane; i < w_lines; i += (size_t)total_w * 32)
       asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_W + (i << 7)));
-    for (int h = 0; h < P.Hq; ++h)
-      for (size_t i = (size_t)gw * 32 + lane; i < r_lines; i += (size_t)total_w * 32)
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_route + (size_t)h * P.route_head_stride * 2 + (i << 7)));
+    for (size_t i = (size_t)gw * 32 + lane; i < r_lines * P.Hq; i += (size_t)total_w * 32) {
+      const size_t h = i / r_lines, li = i - h * r_lines;
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_route + h * P.route_head_stride * 2 + (li << 7)));
+    }
   }
   // last CTA out re-arms the queues and counters and advances the layer's step stamp
   __syncthreads();
@@ -1390,15 +1396,21 @@ int fused_warps(const sekv_handle* h) {
 }
 
 template <int G>
-static cudaError_t launch_fused_g(const FusedParams& P, size_t smem, int grid, int threads, cudaStream_t s) {
+static cudaError_t launch_fused_g(const FusedParams& P, size_t smem, int grid, int threads, cudaStream_t s, bool pdl) {
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  fused_layer_kernel<G><<<grid, threads, smem, s>>>(P);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, fused_layer_kernel<G>, P);
 }
 
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
@@ -1447,14 +1459,14 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   const int grid = h->fused_grid, threads = 32 * h->fused_warps;
   cudaError_t e;
   switch (h->G) {
-    case 1: e = launch_fused_g<1>(P, smem, grid, threads, s); break;
-    case 2: e = launch_fused_g<2>(P, smem, grid, threads, s); break;
-    case 3: e = launch_fused_g<3>(P, smem, grid, threads, s); break;
-    case 4: e = launch_fused_g<4>(P, smem, grid, threads, s); break;
-    case 5: e = launch_fused_g<5>(P, smem, grid, threads, s); break;
-    case 6: e = launch_fused_g<6>(P, smem, grid, threads, s); break;
-    case 7: e = launch_fused_g<7>(P, smem, grid, threads, s); break;
-    case 8: e = launch_fused_g<8>(P, smem, grid, threads, s); break;
+    case 1: e = launch_fused_g<1>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 2: e = launch_fused_g<2>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 3: e = launch_fused_g<3>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 4: e = launch_fused_g<4>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 5: e = launch_fused_g<5>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 6: e = launch_fused_g<6>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 7: e = launch_fused_g<7>(P, smem, grid, threads, s, h->use_pdl); break;
+    case 8: e = launch_fused_g<8>(P, smem, grid, threads, s, h->use_pdl); break;
     default: return cudaErrorInvalidValue;
   }
   h->launches += 1;

@@ -269,6 +269,7 @@ sekv_status sekv_create(const sekv_config* cfg, void* device_arena, size_t devic
   h->launches = 0;
   h->profiling = false;
   h->trace_buf = nullptr; h->trace_cap = 0;
+  h->use_pdl = true;
   *out = h;
   sekv_status s = sekv_reset(h);
   if (s != SEKV_OK) { sekv_destroy(h); *out = nullptr; return s; }
@@ -784,12 +785,17 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   if (e != cudaSuccess || e2 != cudaSuccess) {
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
+    if (h->use_pdl) { h->use_pdl = false; return sekv_decode_step(h, q, tau, k, out, lse); }   // retry without the PDL edges
     return cuda_fail(h, e != cudaSuccess ? e : e2, "decode_step graph capture");
   }
   GraphEntry ge{q, tau, k, out, lse, nullptr, nodes};
   cudaError_t e3 = cudaGraphInstantiate(&ge.exec, graph, 0);
   cudaGraphDestroy(graph);
-  if (e3 != cudaSuccess) return cuda_fail(h, e3, "cudaGraphInstantiate");
+  if (e3 != cudaSuccess) {
+    cudaGetLastError();
+    if (h->use_pdl) { h->use_pdl = false; return sekv_decode_step(h, q, tau, k, out, lse); }
+    return cuda_fail(h, e3, "cudaGraphInstantiate");
+  }
   if (h->graphs.size() >= 64) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
   h->graphs.push_back(ge);
   CK(h, cudaGraphLaunch(ge.exec, h->main));

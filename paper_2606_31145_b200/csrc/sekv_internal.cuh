@@ -251,7 +251,7 @@ struct sekv_handle {
   // schedule
   int n_chunks, parts1_max, P2, parts_per_head, sort_n;
   // fused layer kernel (bf16 path)
-  bool use_fused;
+  bool use_fused, use_pdl;
   int n_items, n_lat_items, select_begin, pool_end, fused_grid, fused_warps, fused_item_rows;
   int num_sms;
   std::vector<GraphEntry> graphs;
