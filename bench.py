@@ -24,6 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "sekv_decode_attn_us_per_layer_step_128k"
+NCU_DRAM_BYTES_PER_LAUNCH = 123.1e6   # 118.4 MB read + 4.7 MB written (algorithmic: 108.6 MB)
 UNIT = "us/layer-step"
 
 
@@ -279,7 +280,11 @@ def run_ours(args):
     dom_us = max(dom["ms"] * 1e3 / max(1, dom["launches"]), 1e-9)
     roofline = {"bound": "hbm", "kernel": dom_name,
                 "achieved": dom_bytes / (dom_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
-                "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak,
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch of the layer kernel, from the one
+                # `ncu --set full` capture summarised in profiles/r01_fused_layer_kernel_ncu_full.md
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if kt["fused"]["launches"] and not args.layers and args.config == 2 else None,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_us": dom_us,
                 "share_of_step_kernel_time": dom["ms"] / max(1e-9, tot_kernel_ms),
                 "timing": "CUDA events on the launching stream around every launch, eager launches, %d steps" % args.profile_steps,

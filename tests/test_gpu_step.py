@@ -101,3 +101,33 @@ def test_step_small_cache_evicts_lru():
     eng, st, _ = _run_steps(spec, 4, 0.3, heads=[1, 18], prefetch=2, cache_ways=18)
     assert st["cache_misses"] > 8 * 16
     eng.close()
+
+
+def test_item_trace_records_every_work_item():
+    """sekv_set_trace: one 64-byte record per work item of a layer launch (plus one per group for the team's
+    selection / plan), begin <= wait mark <= end, known kinds; switching it off leaves the outputs unchanged."""
+    from paper_2606_31145_b200 import engine as E
+    spec = get_spec(1).sharp().with_(contexts=(12000,))
+    lay = make_layouts(spec)
+    eng = E.create_engine(spec, lay)
+    q = make_queries(spec, 0, "cuda")
+    out0 = torch.zeros((1, 1, spec.n_q_heads, 128), dtype=torch.float32, device="cuda")
+    out1 = torch.zeros_like(out0)
+    eng.sekv_decode_step(q, spec.top_k, out0)
+    buf = torch.zeros(16384 * 8, dtype=torch.int64, device="cuda")
+    n = eng.sekv_set_trace(buf)
+    assert n > 0
+    eng.sekv_decode_step(q, spec.top_k, out1)
+    torch.cuda.synchronize()
+    groups = spec.batch * spec.n_kv_heads
+    r = buf.cpu().numpy().reshape(-1, 8)
+    rec = r[:n + groups]
+    kind = rec[:, 0] & 0xFFFFFFFF
+    assert (rec[:, 3] >= rec[:, 2]).all() and (rec[:, 2] > 0).all(), "every item has begin <= end stamps"
+    assert (rec[:, 4] >= rec[:, 2]).all() and (rec[:, 4] <= rec[:, 3]).all(), "wait mark inside the item"
+    assert set(int(k) for k in kind) <= set(range(7))
+    assert int((kind == 2).sum()) == groups                     # one selection / plan per (sequence, kv head)
+    assert (r[n + groups:] == 0).all()
+    assert eng.sekv_set_trace(None) == n
+    assert torch.equal(out0, out1)
+    eng.close()
