@@ -524,7 +524,8 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
   uint32_t* keys = reinterpret_cast<uint32_t*>(region);
   uint32_t* hist = reinterpret_cast<uint32_t*>(region + P.sm_hist);
   unsigned long long* cand = reinterpret_cast<unsigned long long*>(region + P.sm_cand);
-  int* sel = T.scratch + 8;                                    // [0] digit, [1] keys above it, [2..4] ne / kmin / kmax
+  int* sel = T.scratch + 8;                // [0] digit, [1] keys above it, [2..4] ne / kmin / kmax, [5] keys == T, [6] slot
+  for (int i = T.tt; i < 4 * 256; i += T.ts) hist[i] = 0u;     // one histogram per radix pass, zeroed while waiting
   const uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
   const int n_route = (m + P.route_spans - 1) / P.route_spans;
   if (T.tt == 0) {
@@ -536,7 +537,7 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
       __nanosleep(64);
     }
     (void)ld_acquire(reinterpret_cast<const uint32_t*>(c));
-    sel[2] = 0; sel[3] = -1; sel[4] = 0;
+    sel[2] = 0; sel[3] = -1; sel[4] = 0; sel[5] = 0; sel[6] = 0;
     mark(tm, 0, 0);
   }
   team_bar(T);
@@ -584,22 +585,21 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
     uint32_t maskb = (top + 8 >= 32) ? 0u : ~((1u << (top + 8)) - 1u);
     uint32_t prefix = kmax & maskb;
     need = n_cand;
-    for (int shift = top; shift >= 0; shift = (shift >= 8 ? shift - 8 : (shift > 0 ? 0 : -1))) {
-      for (int i = T.tt; i < 256; i += T.ts) hist[i] = 0u;
-      team_bar(T);
+    uint32_t* hp = hist;
+    for (int shift = top; shift >= 0; shift = (shift >= 8 ? shift - 8 : (shift > 0 ? 0 : -1)), hp += 256) {
       for (int i = T.tt; i < m; i += T.ts) {
         const uint32_t k = keys[i];
-        if (k != 0u && (k & maskb) == prefix) atomicAdd(&hist[(k >> shift) & 255u], 1u);
+        if (k != 0u && (k & maskb) == prefix) atomicAdd(&hp[(k >> shift) & 255u], 1u);
       }
       team_bar(T);
       if (T.tw == 0) {
         int loc[8], tot = 0;
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { loc[e] = (int)hist[255 - (8 * T.lane + e)]; tot += loc[e]; }
+        for (int e = 0; e < 8; ++e) { loc[e] = (int)hp[255 - (8 * T.lane + e)]; tot += loc[e]; }
         int run = warp_excl_scan(tot, T.lane);     // matching keys in bins above this lane's bins
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-          if (run < need && run + loc[e] >= need) { sel[0] = 255 - (8 * T.lane + e); sel[1] = run; }
+          if (run < need && run + loc[e] >= need) { sel[0] = 255 - (8 * T.lane + e); sel[1] = run; sel[5] = loc[e]; }
           run += loc[e];
         }
       }
@@ -611,6 +611,20 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
     Tk = prefix;
   }
   mark(tm, 2, T.tt);
+  const bool cut_ties = (n_cand != 0 && n_cand < n_elig) && sel[5] != need;   // more keys == T than are taken
+  if (!cut_ties) {
+    // every key >= T is taken: append in any order (the sort below fixes the order)
+    const uint32_t lo_key = (n_cand != 0 && n_cand < n_elig) ? Tk : (n_cand == 0 ? 0xFFFFFFFFu : 1u);
+    if (n_cand != 0)
+      for (int i = T.tt; i < m; i += T.ts) {
+        const uint32_t k = keys[i];
+        if (k >= lo_key) {
+          const int pos = atomicAdd(&sel[6], 1);
+          if (pos < P.kc) cand[pos] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
+        }
+      }
+    team_bar(T);
+  } else {
   // ordered compaction: each thread owns a contiguous block of span ids
   const int per = (m + T.ts - 1) / T.ts;
   const int lo = min(m, T.tt * per), hi = min(m, lo + per);
@@ -628,6 +642,7 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
     if (s && pos < P.kc) cand[pos++] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
   }
   team_bar(T);
+  }
   if (n_cand <= T.ts) {
     if (T.tt < n_cand) {
       const unsigned long long mine = cand[T.tt];
@@ -1361,7 +1376,7 @@ size_t fused_plan_smem(const sekv_handle* h, FusedParams* P) {
   const sekv_config& c = h->cfg;
   const int kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
   size_t o = (size_t)round_up(std::max(h->max_m, 1), 4) * 4;             // keys
-  o = round_up_sz(o, 16); P->sm_hist = (int)o; o += 256 * 4;
+  o = round_up_sz(o, 16); P->sm_hist = (int)o; o += 4 * 256 * 4;
   o = round_up_sz(o, 16); P->sm_cand = (int)o; o += (size_t)pow2_ceil(std::max(kc, 64)) * 8;
   o = round_up_sz(o, 16); P->sm_ids = (int)o; o += (size_t)kc * 4;
   o = round_up_sz(o, 16); P->sm_wayof = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 8) * 2;
