@@ -907,31 +907,41 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
   float yf[2 * NK][4];
 #pragma unroll
   for (int n = 0; n < 2 * NK; ++n) { yf[n][0] = yf[n][1] = yf[n][2] = yf[n][3] = 0.f; }
-  for (int grp = 0; grp < ngrp; ++grp) {
-    const uint8_t* UKc = blob + bd.off_chunks + (size_t)grp * bd.chunk_bytes;
-    const uint8_t* UVtc = UKc + bd.uvt_in_chunk;
-    float sacc[2][4];
+  // two 16-token chunks per iteration: their logits are independent, one running-max update serves both
+  for (int grp = 0; grp < ngrp; grp += 2) {
+    const bool two = grp + 1 < ngrp;
+    float sacc[2][2][4];
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      sacc[u][0] = sacc[u][1] = sacc[u][2] = sacc[u][3] = 0.f;
-      const uint8_t* prow = UKc + (size_t)pi_index(u, gid) * (bd.rkp * 2) + t4 * 8;
+    for (int cc = 0; cc < 2; ++cc) {
+      const uint8_t* UKc = blob + bd.off_chunks + (size_t)(grp + cc) * bd.chunk_bytes;
 #pragma unroll
-      for (int ks = 0; ks < NK; ++ks) {
-        if (ks < nks) {
-          uint2 bv = make_uint2(0u, 0u);
-          if (16 * ks + 4 * t4 < bd.rkp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
-          mma16816(sacc[u], ckh[ks][0], ckh[ks][1], bv.x, bv.y);
-          mma16816(sacc[u], ckl[ks][0], ckl[ks][1], bv.x, bv.y);
+      for (int u = 0; u < 2; ++u) {
+        sacc[cc][u][0] = sacc[cc][u][1] = sacc[cc][u][2] = sacc[cc][u][3] = 0.f;
+        const uint8_t* prow = UKc + (size_t)pi_index(u, gid) * (bd.rkp * 2) + t4 * 8;
+#pragma unroll
+        for (int ks = 0; ks < NK; ++ks) {
+          if (ks < nks) {
+            uint2 bv = make_uint2(0u, 0u);
+            if ((cc == 0 || two) && 16 * ks + 4 * t4 < bd.rkp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
+            mma16816(sacc[cc][u], ckh[ks][0], ckh[ks][1], bv.x, bv.y);
+            mma16816(sacc[cc][u], ckl[ks][0], ckl[ks][1], bv.x, bv.y);
+          }
         }
       }
     }
-    // this lane: head gid, tokens 16grp + 4*t4 + 2u + e
-    float z[2][2];
+    // this lane: head gid, tokens 16 (grp + cc) + 4*t4 + 2u + e
+    float z[2][2][2];
+    float mx = -INFINITY;
 #pragma unroll
-    for (int u = 0; u < 2; ++u)
+    for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
-      for (int e = 0; e < 2; ++e) z[u][e] = (16 * grp + 4 * t4 + 2 * u + e < bd.len) ? sacc[u][e] : -INFINITY;
-    const float mx = quad_max(fmaxf(fmaxf(z[0][0], z[0][1]), fmaxf(z[1][0], z[1][1])));
+      for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          z[cc][u][e] = (16 * (grp + cc) + 4 * t4 + 2 * u + e < bd.len) ? sacc[cc][u][e] : -INFINITY;
+          mx = fmaxf(mx, z[cc][u][e]);
+        }
+    mx = quad_max(mx);
     const float m_new = fmaxf(m_s, mx);
     const float m_safe = (m_new == -INFINITY) ? 0.f : m_new;
     if (__any_sync(0xffffffffu, m_new > m_s)) {
@@ -941,21 +951,26 @@ __device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDi
       for (int n = 0; n < 2 * NK; ++n) { yf[n][0] *= corr; yf[n][1] *= corr; }
     }
     m_s = m_new;
-    const float p00 = exp2f(z[0][0] - m_safe), p01 = exp2f(z[0][1] - m_safe);
-    const float p10 = exp2f(z[1][0] - m_safe), p11 = exp2f(z[1][1] - m_safe);
-    l_s += (p00 + p01) + (p10 + p11);
-    uint32_t a0h, a0l, a2h, a2l;
-    split_bf16(p00, p01, a0h, a0l);     // tokens 4*t4 + {0,1}  <-> k = 2*t4 + e
-    split_bf16(p10, p11, a2h, a2l);     // tokens 4*t4 + {2,3}  <-> k = 8 + 2*t4 + e
-    // y += P U_V : B[k = token][n = i] read from the transposed factor UVt[i][token]
 #pragma unroll
-    for (int n = 0; n < 2 * NK; ++n) {
-      if (n < 2 * nvs) {
-        const int irow = pi_index(n, gid);
-        uint2 bv = make_uint2(0u, 0u);
-        if (irow < bd.rvp) bv = *reinterpret_cast<const uint2*>(UVtc + (size_t)irow * (kLenPad * 2) + t4 * 8);
-        mma16816(yf[n], a0h, a2h, bv.x, bv.y);
-        mma16816(yf[n], a0l, a2l, bv.x, bv.y);
+    for (int cc = 0; cc < 2; ++cc) {
+      if (cc == 1 && !two) break;
+      const uint8_t* UVtc = blob + bd.off_chunks + (size_t)(grp + cc) * bd.chunk_bytes + bd.uvt_in_chunk;
+      const float p00 = exp2f(z[cc][0][0] - m_safe), p01 = exp2f(z[cc][0][1] - m_safe);
+      const float p10 = exp2f(z[cc][1][0] - m_safe), p11 = exp2f(z[cc][1][1] - m_safe);
+      l_s += (p00 + p01) + (p10 + p11);
+      uint32_t a0h, a0l, a2h, a2l;
+      split_bf16(p00, p01, a0h, a0l);     // tokens 4*t4 + {0,1}  <-> k = 2*t4 + e
+      split_bf16(p10, p11, a2h, a2l);     // tokens 4*t4 + {2,3}  <-> k = 8 + 2*t4 + e
+      // y += P U_V : B[k = token][n = i] read from the transposed factor UVt[i][token]
+#pragma unroll
+      for (int n = 0; n < 2 * NK; ++n) {
+        if (n < 2 * nvs) {
+          const int irow = pi_index(n, gid);
+          uint2 bv = make_uint2(0u, 0u);
+          if (irow < bd.rvp) bv = *reinterpret_cast<const uint2*>(UVtc + (size_t)irow * (kLenPad * 2) + t4 * 8);
+          mma16816(yf[n], a0h, a2h, bv.x, bv.y);
+          mma16816(yf[n], a0l, a2l, bv.x, bv.y);
+        }
       }
     }
   }
