@@ -25,14 +25,14 @@ def _run_steps(spec, n_steps, rho, heads=None, **cfg_kw):
              for b in range(eng.n_seqs)] for l in range(spec.n_layers)]
     L, B, Hq, Hkv = spec.n_layers, spec.batch, spec.n_q_heads, spec.n_kv_heads
     q = make_queries(spec, 0, "cuda")
-    out = torch.zeros((L, B, Hq, 128), dtype=torch.float32, device="cuda")
+    out = torch.zeros((L, B, Hq, 128), dtype=eng.out_dtype, device="cuda")
     lse = torch.zeros((L, B, Hq), dtype=torch.float32, device="cuda")
     hs = list(range(Hq)) if heads is None else list(heads)
     worst = dict(rel_l2=0.0, max_abs=0.0, lse=0.0)
     for step in range(n_steps):
         eng.sekv_decode_step(q, spec.top_k, out, lse=lse)
         torch.cuda.synchronize()
-        out_h = out.cpu().numpy().astype(np.float64)
+        out_h = out.float().cpu().numpy().astype(np.float64)
         lse_h = lse.cpu().numpy().astype(np.float64)
         qn = to_np(q)
         for l in range(L):
@@ -100,6 +100,20 @@ def test_step_small_cache_evicts_lru():
     spec = get_spec(1).sharp().with_(contexts=(16000,))
     eng, st, _ = _run_steps(spec, 4, 0.3, heads=[1, 18], prefetch=2, cache_ways=18)
     assert st["cache_misses"] > 8 * 16
+    eng.close()
+
+
+def test_step_config2_full_size_bench_configuration():
+    """configs[2] at its full per-layer size (batch 4 x 128K context, r = 16, top-k = 32) in the launch
+    configuration bench.py times (CUDA graph with programmatic dependent launches, speculative prefetch 8,
+    bf16 output, AR(1) stream with rho = 0.99), two layers built: every step's zoom sets of every (sequence,
+    kv head) and the outputs of a sample of query heads against the oracle."""
+    spec = get_spec(2).with_(n_layers=2)
+    eng, st, worst = _run_steps(spec, 3, 0.99, heads=[0, 5, 18, 31], prefetch=8, use_graph=1, out_dtype="bf16")
+    print("step cfg2", worst, st)
+    assert st["layer_steps"] == 6
+    assert st["zoomed_spans"] == 3 * 2 * 4 * 8 * 32
+    assert st["cache_hits"] > st["cache_misses"] // 2          # steps 2 and 3 reuse most of step 1's factors
     eng.close()
 
 
