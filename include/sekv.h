@@ -269,7 +269,8 @@ SEKV_API sekv_status sekv_set_profiling(sekv_handle* h, int32_t on);
 SEKV_API sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t* launches);
 /* Work-item trace of the fused layer kernel (a debugging and tuning instrument; off by default).
  * `buf` is a DEVICE buffer of capacity_items records of 64 bytes, borrowed until the next call
- * (buf = NULL switches tracing off).  Every launch overwrites record i for work item i with
+ * (buf = NULL switches tracing off).  Every launch of layer l overwrites record l * (*n_items + groups) + i
+ * (groups = sequences x kv heads; the team's selection / plan of group g is item *n_items + g) for work item i with
  * { int32 kind, int32 group, uint16 sm, uint16 warp, int32 0, uint64 t_begin_ns, uint64 t_end_ns,
  *   uint64 mark_ns[4] } (%globaltimer; mark 0 = end of the item's dependency wait);
  * items past the capacity are not recorded.  HOST out *n_items: items per full layer launch. */

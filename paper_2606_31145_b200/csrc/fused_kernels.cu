@@ -1461,7 +1461,12 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.plan_counts = (int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
   P.stats = (unsigned long long*)ws(h, h->F.off_stats);
   P.host_arena = h->host_dev;
-  P.trace = (unsigned long long*)h->trace_buf; P.trace_cap = h->trace_cap;
+  {   // trace records of layer l start at record l * (n_items + groups)
+    const int64_t stride = (int64_t)h->n_items + (int64_t)h->n_seqs * c.n_kv_heads;
+    const int64_t left = h->trace_cap - (int64_t)layer * stride;
+    P.trace = (h->trace_buf && left > 0) ? (unsigned long long*)h->trace_buf + 8 * (size_t)layer * stride : nullptr;
+    P.trace_cap = left > 0 ? std::min(left, stride) : 0;
+  }
   P.mode = mode; P.k = k; P.k_cap = c.k_cap; P.prefetch = std::max(c.prefetch, 0);
   P.kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
   P.BG = h->n_seqs * c.n_kv_heads;
