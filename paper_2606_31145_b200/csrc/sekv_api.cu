@@ -407,7 +407,7 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
   if (nw < 1) return SEKV_OK;                               // blobs too large for shared memory: generic path
   h->fused_warps = nw;
   h->fused_grid = h->num_sms;                               // one resident CTA per SM
-  int rows = c.item_rows > 0 ? c.item_rows : 64;
+  int rows = c.item_rows > 0 ? c.item_rows : 128;
   h->fused_item_rows = rows;
   const int crows = std::min(rows, 64);
   int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 1;
