@@ -53,6 +53,24 @@ def parse():
     return ap.parse_args()
 
 
+def max_over_ranks(value: float, world: int, device) -> float:
+    """Replicas only: the one exchange between ranks is the max of the device-timed
+    interval; the data path has no collective."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_us_per_layer_step(ms: float, steps: int, layers: int, world: int) -> float:
+    """Whole-job metric of N independent replicas: every rank runs `steps` steps of `layers` layer-steps in
+    `ms` (max over ranks), so the job does world x as many layer-steps in that time."""
+    return ms * 1e3 / (steps * layers) / world
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -241,15 +259,11 @@ def run_ours(args):
     e1.record()
     barrier()
     sampler.stop_flag = True
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
     sampler.join(timeout=2)
     st = eng.sekv_get_stats()
     layer_steps = args.steps * L
-    us_layer_step = ms * 1e3 / layer_steps / world          # aggregate over replicas
+    us_layer_step = replica_us_per_layer_step(ms, args.steps, L, world)   # aggregate over replicas
     algo_bytes = layer_steps * static_bytes - st["coarse_rows_skipped"] * 2 * 128 * esz + st["factor_bytes_algo"]
     hbm_gbs = algo_bytes / (ms * 1e-3) / 1e9 * world
     hit = st["cache_hits"] / max(1, st["zoomed_spans"])
@@ -312,10 +326,7 @@ def run_ours(args):
         eng.sekv_decode_step_host(q_host[i], spec.top_k, out_host)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     st_e = eng.sekv_get_stats()
     e2e = {"value": e2e_s * 1e6 / (args.e2e_steps * L) / world, "unit": UNIT,
            "h2d_bytes_per_step": q_host[0].numel() * esz + st_e["h2d_bytes"] // max(1, args.e2e_steps),
