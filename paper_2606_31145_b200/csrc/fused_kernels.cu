@@ -1196,7 +1196,7 @@ __device__ __forceinline__ Item load_item(const Item* p) {
 }
 
 template <int G>
-__global__ void __maxnreg__(224) fused_layer_kernel(const __grid_constant__ FusedParams P) {
+__global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ FusedParams P) {
   extern __shared__ __align__(128) uint8_t dsm[];
   __shared__ uint64_t bars[8];
   __shared__ int last_flag;
