@@ -24,7 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "sekv_decode_attn_us_per_layer_step_128k"
-NCU_DRAM_BYTES_PER_LAUNCH = 123.1e6   # 118.4 MB read + 4.7 MB written (algorithmic: 108.6 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = 122.9e6   # 118.1 MB read + 4.9 MB written (algorithmic: 108.6 MB)
 UNIT = "us/layer-step"
 
 
