@@ -87,8 +87,8 @@ typedef struct sekv_config {
   int32_t prefetch;          /* speculative prefetch depth: after each layer-step the `prefetch` next-best spans by
                                 routing score that are not resident are copied host -> cache on the side stream */
   int32_t stage1_ctas;       /* generic path: stage-1 grid; 0 = auto (multiple of the SM count) */
-  int32_t item_rows;         /* fused path: entry rows per POOL / COARSE work item, multiple of 16; 0 = auto */
-  int32_t zoom_spans_per_item; /* fused path: expanded spans per ZOOM work item; 0 = auto (4) */
+  int32_t item_rows;         /* fused path: entry rows per POOL work item, multiple of 16 (COARSE items: min(this, 64)); 0 = 128 */
+  int32_t zoom_spans_per_item; /* fused path: expanded spans per ZOOM work item; 0 = 1 */
   int32_t use_graph;         /* 1: sekv_decode_step replays a captured CUDA graph */
   int32_t impl;              /* 0 = auto (bf16: the fused layer kernel), 1 = force the generic multi-kernel path */
   void* main_stream;         /* cudaStream_t; NULL = legacy default stream */
