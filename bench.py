@@ -209,12 +209,12 @@ def run_ours(args):
         spec = spec.with_(n_layers=args.layers)
     layouts = make_layouts(spec)
     t_setup = time.time()
-    cfg = E.config_for(spec, layouts, out_dtype="bf16", use_graph=0 if args.no_graph else 1,
-                       impl=1 if args.generic else 0, stage1_ctas=args.stage1_ctas, prefetch=args.prefetch,
-                       cache_ways=args.cache_ways or None, item_rows=args.item_rows,
-                       zoom_spans_per_item=args.zoom_spans)
-    eng = B.Sekv(cfg, E.host_bytes_for(spec, layouts, cfg), device=dev)
-    H_dev = E.surprisal_device(layouts, eng.device)
+    H_dev = E.surprisal_device(layouts, dev)
+    cfg, host_bytes = E.config_for(spec, layouts, out_dtype="bf16", use_graph=0 if args.no_graph else 1,
+                                   impl=1 if args.generic else 0, stage1_ctas=args.stage1_ctas, prefetch=args.prefetch,
+                                   cache_ways=args.cache_ways or None, item_rows=args.item_rows,
+                                   zoom_spans_per_item=args.zoom_spans, H_dev=H_dev, device=dev)
+    eng = B.Sekv(cfg, host_bytes, device=dev)
     for layer in range(spec.n_layers):
         li = make_layer_inputs(spec, layouts, layer, device=dev)
         E.build_layer_prefactored(eng, spec, layouts, li, H_dev)

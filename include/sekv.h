@@ -87,8 +87,8 @@ typedef struct sekv_config {
   int32_t prefetch;          /* speculative prefetch depth: after each layer-step the `prefetch` next-best spans by
                                 routing score that are not resident are copied host -> cache on the side stream */
   int32_t stage1_ctas;       /* generic path: stage-1 grid; 0 = auto (multiple of the SM count) */
-  int32_t item_rows;         /* fused path: entry rows per POOL work item, multiple of 16 (COARSE items: min(this, 64)); 0 = 128 */
-  int32_t zoom_spans_per_item; /* fused path: expanded spans per ZOOM work item; 0 = 1 */
+  int32_t item_rows;         /* fused path: entry rows per POOL work item, multiple of 16 (COARSE items: min(this, 64)); 0 = one round over the streaming warps */
+  int32_t zoom_spans_per_item; /* reserved (the fused path runs one expanded span per ZOOM work item) */
   int32_t use_graph;         /* 1: sekv_decode_step replays a captured CUDA graph */
   int32_t impl;              /* 0 = auto (bf16: the fused layer kernel), 1 = force the generic multi-kernel path */
   void* main_stream;         /* cudaStream_t; NULL = legacy default stream */
@@ -118,7 +118,7 @@ typedef struct sekv_layout {
   int64_t w;                     /* st [L][H][d'][128] */
   int64_t w_layer_stride;
   int64_t dir_off;               /* int64 [L][H_kv][spans_cap] byte offset of the span's blob in the host arena */
-  int64_t dir_rank;              /* int32 [L][H_kv][spans_cap] r_K | r_V << 8 */
+  int64_t dir_rank;              /* int32 [L][H_kv][spans_cap] r_K | r_V << 8 | |S| << 16 */
   int64_t dir_layer_stride_elems;
   /* device factor cache */
   int64_t cache_tags;            /* int32 [L][B][H_kv][ways] span id or -1 */
@@ -135,12 +135,24 @@ typedef struct sekv_stats {
   uint64_t zoomed_spans;         /* (sequence, kv head, span) expansions */
   uint64_t cache_hits;
   uint64_t cache_misses;
-  uint64_t h2d_bytes;            /* factor bytes fetched host -> device cache */
+  uint64_t h2d_bytes;            /* DEMAND-miss factor bytes read from the pinned host store (Eq. 20) */
   uint64_t factor_bytes_algo;    /* sum over expansions of (r_K+r_V)(|S|+d_h) b + 4(r_K+r_V): Eq. 18 with fp32 sigma */
   uint64_t coarse_rows_skipped;  /* coarse entries replaced by their tokens (= zoomed_spans) */
-  uint64_t prefetched_spans;     /* blobs copied by the side-stream prefetch (their bytes are in h2d_bytes) */
+  uint64_t prefetched_spans;     /* blobs copied by the side-stream prefetch (only those that were given a slot) */
   uint64_t kernel_launches;      /* kernels launched or graph nodes replayed by this handle */
+  uint64_t prefetch_h2d_bytes;   /* bytes of the blobs copied by the speculative side-stream prefetch */
 } sekv_stats;
+
+/* Capacities a caller needs BEFORE sekv_create (sekv_build_sizes). */
+typedef struct sekv_sizes {
+  int64_t tokens_total;          /* sum_b n_b */
+  int32_t spans_total;           /* sum_b m_b: exact when H was given, else the bound sum_b floor(n_b / l_min) */
+  int32_t full_total;            /* sum_b A_b: exact when H was given, else the bound sum_b n_b */
+  int32_t max_spans_per_seq;
+  int32_t max_span_len;          /* longest span (exact), else min(SEKV_MAX_SPAN_LEN, longest sequence) */
+  int32_t exact;                 /* 1 when computed from H by the segmentation rule */
+  int64_t host_bytes;            /* pinned factor store: all layers, kv heads and spans at rank min(r_max, |S|) */
+} sekv_sizes;
 
 /* Prefactored build input: the caller supplies the factors instead of dense K/V (skips Eq. 6's
  * SVD; needed to stage 128K x 32 layers where dense K/V would be 68.7 GB).  All DEVICE pointers.
@@ -173,6 +185,16 @@ SEKV_API sekv_status sekv_device_arena_bytes(const sekv_config* cfg, size_t* dev
 /* Bytes one span's factor blob occupies in the host arena / a cache slot (padded layout, see
  * DESIGN.md section 6): ranks padded to 8, |S| padded to 16.  Pure function. */
 SEKV_API size_t sekv_blob_bytes(int32_t dtype, int32_t span_len, int32_t rank_k, int32_t rank_v);
+
+/* Sizes for a batch before any handle exists.  cfg: the static fields (n_layers, heads, dtype, alpha, l_min,
+ * r_max, window; capacities are ignored).  seq_tok_off: HOST int64 [n_seqs+1].  H: DEVICE f32 [sum_n] surprisal, or
+ * NULL.  With H the segmentation rule of sekv_build_spans (L55, L108, Eq. 17) is run on the GPU (temporary
+ * cudaMalloc scratch of ~6 bytes per token, synchronous) and the counts are exact; without it they are upper
+ * bounds from the token counts alone (m_b <= n_b / l_min, A_b <= n_b).  spans_per_seq / pool_per_seq: HOST int32
+ * [n_seqs] outputs (nullable; bounds when H is NULL).  The caller copies spans_total / full_total /
+ * max_span_len (rounded up as it likes) into sekv_config and sizes the pinned host arena with host_bytes. */
+SEKV_API sekv_status sekv_build_sizes(const sekv_config* cfg, int32_t n_seqs, const int64_t* seq_tok_off, const float* H,
+                             sekv_sizes* out, int32_t* spans_per_seq, int32_t* pool_per_seq);
 
 /* device_arena: DEVICE, 256-byte aligned, >= sekv_device_arena_bytes.  host_arena: HOST, pinned and
  * device-mapped (cudaHostAlloc / torch pin_memory), holds the SVD factor store (PAPER.md L106,
@@ -277,6 +299,20 @@ SEKV_API sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t*
 SEKV_API sekv_status sekv_set_trace(sekv_handle* h, void* buf, int64_t capacity_items, int32_t* n_items);
 /* Number of stage-1 work chunks (CTAs) and partial slots per query head; HOST outs. */
 SEKV_API sekv_status sekv_get_schedule(const sekv_handle* h, int32_t* stage1_ctas, int32_t* parts_per_head);
+/* Which kernels the built batch runs on.  *fused = 1: the persistent fused layer kernel (bf16 path, one launch
+ * per layer-step); 0: the generic multi-kernel path, and *reason (a string owned by the handle, valid until the
+ * next build / reset) says why -- fp32 storage, impl = 1, a sequence with too many spans for the team's shared
+ * memory, tables too small, the kernel not resident on this device.  Nothing switches paths silently: callers
+ * that depend on the fused kernel's speed check this after the first sekv_build_spans call.  HOST outs. */
+SEKV_API sekv_status sekv_get_path(const sekv_handle* h, int32_t* fused, const char** reason);
+/* Decode one span's factor blob from the pinned host store into plain row-major fp32 HOST arrays (format
+ * decoding only; the blob layout -- mma fragment order, DESIGN.md section 5 -- lives in one place, the
+ * library).  span is LOCAL to sequence seq.  Outputs (nullable): UK [|S|][r_K], sK [r_K], VtK [r_K][128],
+ * UV [|S|][r_V], sV [r_V], VtV [r_V][128]; *len, *rank_k, *rank_v always.  Call with NULL arrays first to
+ * learn the shapes.  *pad_zero = 1 iff every padding element of the blob is zero. */
+SEKV_API sekv_status sekv_export_span_factors(sekv_handle* h, int32_t layer, int32_t seq, int32_t kv_head, int32_t span,
+                                     int32_t* len, int32_t* rank_k, int32_t* rank_v, float* UK, float* sK,
+                                     float* VtK, float* UV, float* sV, float* VtV, int32_t* pad_zero);
 
 #ifdef __cplusplus
 }

@@ -50,11 +50,17 @@ class sekv_layout(C.Structure):
 
 
 _STATS_FIELDS = ["layer_steps", "zoomed_spans", "cache_hits", "cache_misses", "h2d_bytes", "factor_bytes_algo",
-                 "coarse_rows_skipped", "prefetched_spans", "kernel_launches"]
+                 "coarse_rows_skipped", "prefetched_spans", "kernel_launches", "prefetch_h2d_bytes"]
 
 
 class sekv_stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in _STATS_FIELDS]
+
+
+class sekv_sizes(C.Structure):
+    _fields_ = [("tokens_total", C.c_int64), ("spans_total", C.c_int32), ("full_total", C.c_int32),
+                ("max_spans_per_seq", C.c_int32), ("max_span_len", C.c_int32), ("exact", C.c_int32),
+                ("host_bytes", C.c_int64)]
 
 
 class sekv_factors(C.Structure):
@@ -98,12 +104,16 @@ def _load() -> C.CDLL:
     lib.sekv_set_profiling.argtypes = [VP, I32]
     lib.sekv_get_kernel_times.argtypes = [VP, P(C.c_double), P(C.c_uint64)]
     lib.sekv_set_trace.argtypes = [VP, VP, I64, P(I32)]
+    lib.sekv_build_sizes.argtypes = [P(sekv_config), I32, P(I64), VP, P(sekv_sizes), P(I32), P(I32)]
+    lib.sekv_get_path.argtypes = [VP, P(I32), P(C.c_char_p)]
+    lib.sekv_export_span_factors.argtypes = [VP, I32, I32, I32, I32, P(I32), P(I32), P(I32), VP, VP, VP, VP, VP, VP, P(I32)]
     for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
                  "sekv_last_zoom_ids",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
                  "sekv_static_bytes_per_layer", "sekv_get_schedule", "sekv_set_profiling",
-                 "sekv_get_kernel_times", "sekv_set_trace"):
+                 "sekv_get_kernel_times", "sekv_set_trace", "sekv_build_sizes", "sekv_get_path",
+                 "sekv_export_span_factors"):
         getattr(lib, name).restype = C.c_int
     return lib
 
@@ -129,6 +139,22 @@ def sekv_device_arena_bytes(cfg: sekv_config):
     if st != SEKV_OK:
         raise SekvError(st, "sekv_device_arena_bytes")
     return int(dev.value), int(slot.value)
+
+
+def sekv_build_sizes(cfg: sekv_config, seq_tok_off: Sequence[int], H: Optional[torch.Tensor] = None):
+    """(sekv_sizes, spans_per_seq, pool_per_seq) for a batch before any handle exists: exact when the DEVICE
+    surprisal tensor H is given (the segmentation rule runs on the GPU), upper bounds from token counts otherwise."""
+    n = len(seq_tok_off) - 1
+    off = (C.c_int64 * (n + 1))(*[int(x) for x in seq_tok_off])
+    out = sekv_sizes()
+    spans, pool = (C.c_int32 * n)(), (C.c_int32 * n)()
+    if H is not None:
+        assert H.is_cuda and H.dtype == torch.float32 and H.is_contiguous()
+        torch.cuda.synchronize(H.device)
+    st = lib.sekv_build_sizes(C.byref(cfg), n, off, None if H is None else H.data_ptr(), C.byref(out), spans, pool)
+    if st != SEKV_OK:
+        raise SekvError(st, "sekv_build_sizes")
+    return out, list(spans), list(pool)
 
 
 def make_config(**kw) -> sekv_config:
@@ -331,6 +357,30 @@ class Sekv:
         self._check(lib.sekv_set_trace(self._h, _ptr(buf), cap, C.byref(n)), "sekv_set_trace")
         self._trace_buf = buf
         return int(n.value)
+
+    def sekv_get_path(self):
+        """(fused, reason): whether the built batch runs on the fused layer kernel, and why not if it does not."""
+        f, why = C.c_int32(0), C.c_char_p(None)
+        self._check(lib.sekv_get_path(self._h, C.byref(f), C.byref(why)), "sekv_get_path")
+        return bool(f.value), (why.value or b"").decode()
+
+    def sekv_export_span_factors(self, layer: int, seq: int, kv_head: int, span: int) -> dict:
+        """One span's factors decoded by the library into row-major float32 numpy arrays."""
+        import numpy as np
+        ln, rk, rv, pad = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)
+        st = lib.sekv_export_span_factors(self._h, layer, seq, kv_head, span, C.byref(ln), C.byref(rk), C.byref(rv),
+                                          None, None, None, None, None, None, None)
+        self._check(st, "sekv_export_span_factors")
+        n, a, b = ln.value, rk.value, rv.value
+        arr = dict(UK=np.zeros((n, a), np.float32), sK=np.zeros(a, np.float32), VtK=np.zeros((a, 128), np.float32),
+                   UV=np.zeros((n, b), np.float32), sV=np.zeros(b, np.float32), VtV=np.zeros((b, 128), np.float32))
+        ptr = lambda x: x.ctypes.data_as(C.c_void_p)
+        st = lib.sekv_export_span_factors(self._h, layer, seq, kv_head, span, C.byref(ln), C.byref(rk), C.byref(rv),
+                                          ptr(arr["UK"]), ptr(arr["sK"]), ptr(arr["VtK"]), ptr(arr["UV"]),
+                                          ptr(arr["sV"]), ptr(arr["VtV"]), C.byref(pad))
+        self._check(st, "sekv_export_span_factors")
+        arr["pad_ok"] = bool(pad.value)
+        return arr
 
     def sekv_get_schedule(self):
         a, b = C.c_int32(0), C.c_int32(0)

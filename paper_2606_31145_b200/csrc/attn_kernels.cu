@@ -167,8 +167,6 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
     const uint8_t* blob = lv.slots + ((size_t)bg * ways + way) * slot_bytes;
     const float* sK = (const float*)(blob + bd.off_sk);
     const float* sV = (const float*)(blob + bd.off_sv);
-    const ST* VtK = (const ST*)(blob + bd.off_vtk);
-    const ST* VV = (const ST*)(blob + bd.off_vv);
     const int es = (int)sizeof(ST);
     // c[h][i]
     for (int o = tid; o < G * bd.rkp; o += kS2Threads) {
@@ -176,7 +174,7 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
       float a = 0.f;
       for (int d = 0; d < kD; d += 4) {
         float v4[4];
-        ld4(VtK + (size_t)i * kD + d, v4);
+        ld4((const ST*)(blob + blob_vtk_off(bd, es, i, d)), v4);
         a = fmaf(v4[0], sh_q[h][d], a); a = fmaf(v4[1], sh_q[h][d + 1], a);
         a = fmaf(v4[2], sh_q[h][d + 2], a); a = fmaf(v4[3], sh_q[h][d + 3], a);
       }
@@ -237,29 +235,20 @@ stage2_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ count, const
     for (int o = tid; o < G * bd.rvp; o += kS2Threads) {
       const int h = o / bd.rvp, i = o % bd.rvp;
       float a = 0.f;
-      for (int t = 0; t < bd.lenp; t += 4) {
-        float u4[4];
-        ld4((const ST*)(blob + blob_uv_off(bd, es, t, i)), u4);
-        a = fmaf(u4[0], sh_z[h][t], a); a = fmaf(u4[1], sh_z[h][t + 1], a);
-        a = fmaf(u4[2], sh_z[h][t + 2], a); a = fmaf(u4[3], sh_z[h][t + 3], a);
-      }
+      for (int t = 0; t < bd.lenp; ++t)
+        a = fmaf(StTraits<ST>::ld((const ST*)(blob + blob_uv_off(bd, es, t, i))), sh_z[h][t], a);
       sh_y[h][i] = a * sV[i];
     }
     __syncthreads();
     // o[h][d] += y[h] . VV[d]
     {
-      const ST* vrow = VV + (size_t)tid * bd.rvp;
       float add[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) add[h] = 0.f;
-      for (int i = 0; i < bd.rvp; i += 4) {
-        float v4[4];
-        ld4(vrow + i, v4);
+      for (int i = 0; i < bd.rvp; ++i) {
+        const float v = StTraits<ST>::ld((const ST*)(blob + blob_vv_off(bd, es, tid, i)));   // V_V[d = tid][i]
 #pragma unroll
-        for (int h = 0; h < G; ++h) {
-          add[h] = fmaf(v4[0], sh_y[h][i], add[h]); add[h] = fmaf(v4[1], sh_y[h][i + 1], add[h]);
-          add[h] = fmaf(v4[2], sh_y[h][i + 2], add[h]); add[h] = fmaf(v4[3], sh_y[h][i + 3], add[h]);
-        }
+        for (int h = 0; h < G; ++h) add[h] = fmaf(v, sh_y[h][i], add[h]);
       }
 #pragma unroll
       for (int h = 0; h < G; ++h) run_o[h] = fmaf(run_o[h], corr[h], add[h]);

@@ -136,6 +136,21 @@ __global__ void seg_compact_kernel(const int64_t* __restrict__ tok_off, const ui
   }
 }
 
+// The four scan kernels of the segmentation rule on caller-provided scratch (also used by sekv_build_sizes):
+// thresholds, boundary / window flags, run lengths (spans vs short runs), per-sequence counts.
+cudaError_t segment_scan(const float* H, int n_seqs, const int64_t* tok_off_dev, double alpha, int window, int l_min,
+                         int max_span_len, uint8_t* flag, uint8_t* flag2, int32_t* len_at, double* thr,
+                         int32_t* counts, int* err, cudaStream_t s) {
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(err, 0, 4, s)) != cudaSuccess) return e;
+  seg_threshold_kernel<<<n_seqs, 1024, 0, s>>>(H, tok_off_dev, alpha, thr);
+  dim3 grid(64, n_seqs);
+  seg_flag_kernel<<<grid, 256, 0, s>>>(H, tok_off_dev, thr, window, flag, flag2);
+  seg_runs_kernel<<<grid, 256, 0, s>>>(tok_off_dev, flag, flag2, len_at, l_min, max_span_len, err);
+  seg_count_kernel<<<n_seqs, 1024, 0, s>>>(tok_off_dev, flag2, counts);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_segment(sekv_handle* h, const float* H, int n_seqs, const int64_t* tok_off_host, int* m_out,
                            int* a_out, std::string* why) {
   const sekv_config& c = h->cfg;
@@ -149,14 +164,9 @@ cudaError_t launch_segment(sekv_handle* h, const float* H, int n_seqs, const int
   int32_t* counts = (int32_t*)(ws(h, h->F.off_seg_misc) + (size_t)c.max_seqs * 8);
   int* err = (int*)ws(h, h->F.off_err_flag);
   if ((e = cudaMemcpyAsync((void*)cv.seq_tok_off, tok_off_host, (size_t)(n_seqs + 1) * 8, cudaMemcpyHostToDevice, s)) != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(err, 0, 4, s)) != cudaSuccess) return e;
-  seg_threshold_kernel<<<n_seqs, 1024, 0, s>>>(H, cv.seq_tok_off, (double)c.alpha, thr);
-  dim3 grid(64, n_seqs);
-  seg_flag_kernel<<<grid, 256, 0, s>>>(H, cv.seq_tok_off, thr, c.window, flag, flag2);
-  seg_runs_kernel<<<grid, 256, 0, s>>>(cv.seq_tok_off, flag, flag2, len_at, c.l_min, c.max_span_len, err);
-  seg_count_kernel<<<n_seqs, 1024, 0, s>>>(cv.seq_tok_off, flag2, counts);
+  if ((e = segment_scan(H, n_seqs, cv.seq_tok_off, (double)c.alpha, c.window, c.l_min, c.max_span_len, flag, flag2,
+                        len_at, thr, counts, err, s)) != cudaSuccess) return e;
   h->launches += 4;
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
   std::vector<int32_t> cnt((size_t)n_seqs * 2);
   int herr = 0;
   if ((e = cudaMemcpyAsync(cnt.data(), counts, cnt.size() * 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
@@ -346,28 +356,38 @@ __global__ void pack_blob_kernel(CsrView cv, sekv_factors f, size_t tok_tot, int
   for (int i = tid; i < bd.rkp; i += nt) bsk[i] = i < rk ? SK[i] : 0.f;
   for (int i = tid; i < bd.rvp; i += nt) bsv[i] = i < rv ? SV[i] : 0.f;
   const ST zero = ST(0.f);
-  // VtK [rkp][128]
+  // The loops run over the DESTINATION in address order (coalesced writes to the mapped host store) and invert
+  // the fragment-order maps of blob_vtk_off / blob_vv_off / blob_uk_off / blob_uv_off (sekv_internal.cuh).
   const ST* vtk = (const ST*)f.VtK + ((size_t)g * m_tot + s) * r * kD;
   ST* bvtk = (ST*)(blob + bd.off_vtk);
-  for (int o = tid; o < bd.rkp * kD; o += nt) { int i = o / kD; bvtk[o] = i < rk ? vtk[o] : zero; }
-  // VV [128][rvp] = transpose of VtV [r][128]
+  for (int o = tid; o < bd.rkp * kD; o += nt) {
+    const int e8 = o & 7, lane = (o >> 3) & 31, blk = o >> 8;
+    const int jj = blk & 3, u = (blk >> 2) & 1, ks = blk >> 3, gid = lane >> 2, t4 = lane & 3;
+    const int i = 16 * ks + 4 * (gid >> 1) + 2 * u + (gid & 1), d = 32 * jj + 8 * t4 + e8;
+    bvtk[o] = i < rk ? vtk[(size_t)i * kD + d] : zero;
+  }
   const ST* vtv = (const ST*)f.VtV + ((size_t)g * m_tot + s) * r * kD;
   ST* bvv = (ST*)(blob + bd.off_vv);
-  for (int o = tid; o < kD * bd.rvp; o += nt) { int d = o / bd.rvp, i = o % bd.rvp; bvv[o] = i < rv ? vtv[(size_t)i * kD + d] : zero; }
-  // chunks of 16 tokens: [UK 16 x rkp][UVt rvp x 16]  (UVt = transpose of UV [len][r])
+  for (int o = tid; o < kD * bd.rvp; o += nt) {
+    const int e = o & 1, reg = (o >> 1) & 3, lane = (o >> 3) & 31, blk = o >> 8;
+    const int md = blk & 7, kv = blk >> 3, gid = lane >> 2, t4 = lane & 3, half = reg >> 1, hi = reg & 1;
+    const int d = 16 * md + 8 * hi + gid, i = 16 * kv + 8 * half + 2 * t4 + e;
+    bvv[o] = i < rv ? vtv[(size_t)i * kD + d] : zero;
+  }
   const ST* uk = (const ST*)f.tokUK + ((size_t)g * tok_tot + tok0) * r;
   const ST* uv = (const ST*)f.tokUV + ((size_t)g * tok_tot + tok0) * r;
   const int per_chunk = kLenPad * (bd.rkp + bd.rvp);
   ST* bch = (ST*)(blob + bd.off_chunks);
   for (int o = tid; o < (bd.lenp / kLenPad) * per_chunk; o += nt) {
     const int c = o / per_chunk, w = o % per_chunk;
+    const int r8 = w & 7, lane = (w >> 3) & 31, blk = w >> 8, gid = lane >> 2, t4 = lane & 3;
     ST v = zero;
-    if (w < kLenPad * bd.rkp) {
-      const int t = c * kLenPad + w / bd.rkp, i = w % bd.rkp;
+    if (blk < bd.nks) {
+      const int t = 16 * c + 8 * (r8 >> 2) + gid, i = 16 * blk + 4 * t4 + (r8 & 3);
       if (t < len && i < rk) v = uk[(size_t)t * r + i];
     } else {
-      const int w2 = w - kLenPad * bd.rkp;
-      const int i = w2 / kLenPad, t = c * kLenPad + w2 % kLenPad;
+      const int reg = r8 >> 1, half = reg >> 1, hi = reg & 1;
+      const int t = 16 * c + 8 * half + 2 * t4 + (r8 & 1), i = 16 * (blk - bd.nks) + 8 * hi + gid;
       if (t < len && i < rv) v = uv[(size_t)t * r + i];
     }
     bch[o] = v;

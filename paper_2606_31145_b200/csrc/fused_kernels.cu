@@ -1,30 +1,26 @@
 // The bf16 hot path: ONE persistent kernel per layer-step that runs a1-a7 (Eq. 4, 5, 9, L123,
-// L119-121, Eq. 8).  One CTA per SM; every WARP is an independent worker with a private shared-memory
-// region and pulls work items from two dependency-ordered queues (first item static, then atomic claims
-// two items ahead so neither the claim nor the descriptor load is on the warp's critical path):
+// L119-121, Eq. 8).  One CTA per SM, kFusedWarps warps, every warp with a private shared-memory region.
 //
-//   latency queue (even warps start here)
-//     QPROJ   (b, h)              q' = W q (Eq. 4) on the tensor cores; published through a sentinel, no flag
-//     ROUTE   (b, g, 64 spans)    x = q'.K_bar/sqrt(d') + ln|S|, alpha = sig(x) (Eq. 5), X = max over the group
-//                                 (GQA), ordered 32-bit keys -> global
-//     SELECT  (b, g)              top-k (Eq. 9, cap L123) by a 4-pass radix select on the keys, ties to the lower
-//                                 span id, sorted ids; then the residency plan of the device factor cache (LRU),
-//                                 zoom bit-mask, one descriptor per expanded span
-//   main queue
-//     POOL    (b, g, row range)   online-softmax partial over full-resolution tokens (no dependency): K/V rows
-//                                 stream through a 3-stage cp.async ring (XOR-swizzled, bank-conflict free)
-//     ZOOM    (b, g, plan items)  expanded spans through the factored form; the span's factor blob moves by ONE
-//                                 1-D bulk async copy (TMA engine) into the warp's region -- from its cache slot
-//                                 on a hit, straight from the pinned-host store over PCIe on a demand miss (and is
-//                                 then written to the slot)
-//     COARSE  (b, g, row range)   partial over the unexpanded coarse entries (+ln|S|); needs the zoom mask
-//     COMBINE (b, h)              log-sum-exp merge of the head's partials -> output (a7)
+//   chain (a1-a4), per (sequence, kv head) group bg, by a TEAM of warps of CTA bg % grid, entirely in
+//   shared memory (no global round trips between the steps):
+//     q' = W q (Eq. 4, tensor cores)  ->  x = q'.K_bar/sqrt(d') + ln|S|, X = max over the group (Eq. 5, GQA;
+//     the routing table streams through a cp.async double buffer)  ->  top-k by radix select (Eq. 9, cap
+//     L123; ties to the lower span id)  ->  residency plan of the device factor cache (LRU), zoom bit-mask,
+//     one stamped descriptor per expanded span
+//   work items (a5-a7), one warp each, claimed in queue order:
+//     POOL    (b, g, rows)   online-softmax partial over full-resolution tokens; no dependency
+//     COARSE  (b, g, rows)   partial over the coarse entries (+ln|S|) of the spans that are NOT expanded
+//                            (an expanded span's coarse entry is replaced by its tokens); waits
+//                            for the group's zoom mask
+//     ZOOM    (b, g, spans)  expanded spans through the factored form (Eq. 8 never materialised); waits for
+//                            the span's descriptor; the U factors move by 1-D bulk copies (TMA engine)
+//     COMBINE (b, h)         log-sum-exp merge of the head's partials -> output (L61)
 //
-// Waiting items only ever wait on items earlier in their queue (or in the latency queue), claims are in
-// queue order and the grid is resident (one CTA per SM), so the wait graph is acyclic.
+// Waiting items only wait on the teams (which start at t = 0 and wait on nobody) or on items earlier in the
+// queue; claims are in queue order and the grid is resident (checked on the host): the wait graph is acyclic.
 //
-// Tensor cores: G <= 8 query heads per kv head is far below a tcgen05 tile and the path is HBM-bound, so
-// the heads are the (padded) 16 rows of warp-level mma.sync.m16n8k16 tiles.
+// Tensor cores: G <= 8 query heads per kv head is far below a tcgen05 tile and the path is HBM-bound, so the
+// heads are the (padded) rows / columns of warp-level mma.sync.m16n8k16 tiles.
 #include <algorithm>
 
 #include "mma_common.cuh"
@@ -33,8 +29,11 @@ namespace sekv {
 
 namespace {
 
-constexpr int kStages = 3;                 // ring stages of a rows item (16 rows of K + 16 rows of V each)
+constexpr int kStages = 2;                 // ring stages of a rows item (16 rows of K + 16 rows of V each)
 constexpr int kStageBytes = 2 * 16 * kD * 2;
+constexpr int kFusedWarps = 12;
+constexpr int kFusedThreads = 32 * kFusedWarps;
+constexpr int kRegionBytes = 19200;        // 12 x 19200 + static < 227 KB
 
 // Monotone map float -> uint32 (larger float => larger key); key 0 is free to mean "not eligible".
 __device__ __forceinline__ uint32_t order_key(float x) {
@@ -44,6 +43,9 @@ __device__ __forceinline__ uint32_t order_key(float x) {
 
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst_smem, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -67,10 +69,37 @@ __device__ __forceinline__ int warp_excl_scan(int v, int lane) {
   }
   return s - v;
 }
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// 2^x on the special function unit (one MUFU; 2^-inf = 0)
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// four 8x8 b16 matrices, transposed on the way in (lanes 8j..8j+7 give the row addresses of matrix j)
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+// transpose an 8x8 b16 matrix held one row-pair per lane (C-fragment layout -> B-fragment layout)
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
+  uint32_t d;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+  return d;
+}
+__device__ __forceinline__ uint4 ld_cg16(const void* p) {       // L2-coherent 16-byte load
+  uint4 v;
+  asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
 
 // per-group counters inside P.ctrs
 __device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
-enum { C_EARLY = 0, C_ROUTE = 1, C_ATTN = 2, C_PLAN = 3 };   // C_EARLY: POOL + COARSE items done
+enum { C_EARLY = 0, C_ATTN = 2 };   // C_EARLY: POOL + COARSE items done, C_ATTN: every attention item done
 
 // spin (lane 0) until the counter reaches `target`
 // (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
@@ -87,7 +116,7 @@ __device__ __forceinline__ void wait_ctr(const int32_t* c, int target, int lane,
   }
   __syncwarp();
 }
-// trace mark k (1..3) of the current item (lane 0; tm = null when tracing is off)
+// trace mark k (0..3) of the current item (lane 0; tm = null when tracing is off)
 __device__ __forceinline__ void mark(unsigned long long* tm, int k, int lane) {
   if (tm && lane == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tm[k]));
 }
@@ -98,6 +127,7 @@ __device__ __forceinline__ void signal_ctr(int32_t* c, int lane) {
   if (lane == 0) red_add_release(c, 1);
 }
 
+// Q fragments of the group's heads (rows gid < G; zero rows above): qf[j] = q[gid][8 (t4 + 4 j) .. +7]
 __device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q, int G, int gid, int t4,
                                              uint32_t (&qf)[4][4]) {
 #pragma unroll
@@ -108,181 +138,12 @@ __device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q
   }
 }
 
-constexpr uint32_t kQpSentinel = 0xFFFFFFFFu;   // never produced by the tensor cores (their NaN is 0x7FFFFFFF)
-
 // ---------------------------------------------------------------------------------------------------
-// a1 (Eq. 4): q'_h = W_h q_h for one query head on the tensor cores: the rows of W_h are the M dimension
-// (16 per tile), the group's queries are the 8 columns, column hl of the result is q'_hl.  All loads of
-// W_h (dp x 128 bf16) are in flight at once.  The result is published without a flag: the buffer holds a
-// sentinel bit pattern until the value arrives, and ROUTE items poll the words they need.
+// The team: warps 0 .. ntw-1 of a CTA, meeting on named barrier 1.  Its tables live at the start of the
+// CTA's dynamic shared memory (the regions of the team's own warps), followed by one routing-table staging
+// buffer per team warp.
 // ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void qproj_item(const FusedParams& P, const Item& I, int lane) {
-  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, dp = P.dp, hl = I.a;
-  const int gid = lane >> 2, t4 = lane & 3;
-  uint32_t qf[4][4];
-  load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
-  const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)(g * G + hl) * dp * (kD * 2) + t4 * 16;
-  float* dst = P.qp + ((size_t)bg * G + hl) * dp;
-#pragma unroll 1
-  for (int j0 = 0; j0 < dp; j0 += 32) {
-    uint4 w[2][2][4];
-#pragma unroll
-    for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
-        const int row = j0 + 16 * mt + 8 * hf + gid;
-#pragma unroll
-        for (int jj = 0; jj < 4; ++jj)
-          w[mt][hf][jj] = row < dp ? ldg16(Wh + (size_t)row * (kD * 2) + jj * 64) : make_uint4(0u, 0u, 0u, 0u);
-      }
-#pragma unroll
-    for (int mt = 0; mt < 2; ++mt) {
-      float c[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-      for (int jj = 0; jj < 4; ++jj) {
-        mma16816_full(c, w[mt][0][jj].x, w[mt][1][jj].x, w[mt][0][jj].y, w[mt][1][jj].y, qf[jj][0], qf[jj][1]);
-        mma16816_full(c, w[mt][0][jj].z, w[mt][1][jj].z, w[mt][0][jj].w, w[mt][1][jj].w, qf[jj][2], qf[jj][3]);
-      }
-      if (t4 == (hl >> 1)) {                                     // this lane holds column hl of the tile
-        const int r = j0 + 16 * mt + gid;
-        if (r < dp) dst[r] = (hl & 1) ? c[1] : c[0];
-        if (r + 8 < dp) dst[r + 8] = (hl & 1) ? c[3] : c[2];
-      }
-    }
-  }
-}
-
-// poll four consecutive words of q' until none is the sentinel
-__device__ __forceinline__ float4 poll_qp4(const float* p) {
-  uint4 v;
-  for (;;) {
-    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
-    if (v.x != kQpSentinel && v.y != kQpSentinel && v.z != kQpSentinel && v.w != kQpSentinel) break;
-    __nanosleep(64);
-  }
-  return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a2 + GQA reduce of a3 (Eq. 5, Eq. 9): spans [I.a, I.b) of (b, g).  The G x nsp rows of the routing table
-// (dp bf16 each) are staged into the warp's region by 16-byte cp.async copies, all in flight while the
-// warp polls q'.  Fast path (d' = 32, no threshold, no score outputs): per head, the staged rows are the M
-// dimension of mma tiles, q' (split into bf16 hi + lo, ~16 bits) the columns; 16 spans x 1 head per 4 mma.
-// General path: compact scalar loops from shared memory (the code footprint matters more than the
-// arithmetic here: every item runs this once).
-// ---------------------------------------------------------------------------------------------------
-template <int G>
-__device__ __forceinline__ void route_item(const FusedParams& P, const Item& I, uint8_t* region, int lane,
-                                           unsigned long long* tm) {
-  const int bg = I.bg, g = bg % P.Hkv, dp = P.dp, lpr = dp >> 3;
-  const int gid = lane >> 2, t4 = lane & 3;
-  const int nsp = I.b - I.a;
-  const uint8_t* route = (const uint8_t*)P.lv.route;
-  const int total = nsp * G * lpr;
-#pragma unroll 2
-  for (int i = lane; i < total; i += 32) {
-    const int c = i % lpr, t = i / lpr;
-    const int hl = t / nsp, s = t - hl * nsp;
-    cp_async16(region + (size_t)i * 16,
-               route + ((size_t)(g * G + hl) * P.route_head_stride + (size_t)(I.span0 + I.a + s) * dp) * 2 + c * 16);
-  }
-  cp_async_commit();
-  const float inv_sqrt_dp = rsqrtf((float)dp);
-  uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
-  const float* gqp = P.qp + (size_t)bg * G * dp;
-  if (dp == 32 && P.tau == nullptr && P.logits_out == nullptr && P.alpha_out == nullptr) {
-    uint32_t bh[4] = {0u, 0u, 0u, 0u}, bl[4] = {0u, 0u, 0u, 0u};
-    float lnl[4];                                                // ln|S| of span 16 i + gid + 8 (t4 & 1)
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int s = 16 * i + gid + 8 * (t4 & 1);
-      lnl[i] = s < nsp ? P.cv.ln_len[I.span0 + I.a + s] : 0.f;
-    }
-    if (gid < G) {
-      const float4 v0 = poll_qp4(gqp + gid * 32 + 8 * t4), v1 = poll_qp4(gqp + gid * 32 + 8 * t4 + 4);
-      split_bf16(v0.x * inv_sqrt_dp, v0.y * inv_sqrt_dp, bh[0], bl[0]);
-      split_bf16(v0.z * inv_sqrt_dp, v0.w * inv_sqrt_dp, bh[1], bl[1]);
-      split_bf16(v1.x * inv_sqrt_dp, v1.y * inv_sqrt_dp, bh[2], bl[2]);
-      split_bf16(v1.z * inv_sqrt_dp, v1.w * inv_sqrt_dp, bh[3], bl[3]);
-    }
-    __syncwarp();
-    mark(tm, 0, lane);
-    cp_async_wait<0>();
-    __syncwarp();
-    mark(tm, 1, lane);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int s0 = 16 * i;
-      if (s0 >= nsp) break;
-      float Xa = -INFINITY, Xb = -INFINITY;                      // spans s0 + gid and s0 + gid + 8
-#pragma unroll
-      for (int hl = 0; hl < G; ++hl) {
-        const uint8_t* ra = region + ((size_t)hl * nsp + s0 + gid) * 64 + t4 * 16;
-        const uint4 a = *reinterpret_cast<const uint4*>(ra), c8 = *reinterpret_cast<const uint4*>(ra + 8 * 64);
-        float c[4] = {0.f, 0.f, 0.f, 0.f};
-        mma16816_full(c, a.x, c8.x, a.y, c8.y, bh[0], bh[1]);
-        mma16816_full(c, a.z, c8.z, a.w, c8.w, bh[2], bh[3]);
-        mma16816_full(c, a.x, c8.x, a.y, c8.y, bl[0], bl[1]);
-        mma16816_full(c, a.z, c8.z, a.w, c8.w, bl[2], bl[3]);
-        if (t4 == (hl >> 1)) {                                   // this lane holds column hl
-          Xa = fmaxf(Xa, (hl & 1) ? c[1] : c[0]);
-          Xb = fmaxf(Xb, (hl & 1) ? c[3] : c[2]);
-        }
-      }
-      Xa = quad_max(Xa); Xb = quad_max(Xb);
-      const int s = s0 + gid + 8 * (t4 & 1);
-      if (t4 < 2 && s < nsp) gkeys[I.a + s] = order_key(((t4 & 1) ? Xb : Xa) + lnl[i]);
-    }
-    mark(tm, 2, lane);
-    signal_ctr(grp_ctr(P, bg, C_ROUTE), lane);
-    return;
-  }
-  float* sqp = reinterpret_cast<float*>(region + (size_t)P.route_spans * G * dp * 2);     // [G][dp]
-  for (int i = 4 * lane; i < G * dp; i += 128) *reinterpret_cast<float4*>(sqp + i) = poll_qp4(gqp + i);
-  mark(tm, 0, lane);
-  cp_async_wait<0>();
-  __syncwarp();
-  mark(tm, 1, lane);
-  for (int s = lane; s < nsp; s += 32) {
-    const float lnl = P.cv.ln_len[I.span0 + I.a + s];
-    float X = -INFINITY;
-    bool elig = (P.tau == nullptr);
-#pragma unroll 1
-    for (int hl = 0; hl < G; ++hl) {
-      const uint4* row = reinterpret_cast<const uint4*>(region + ((size_t)hl * nsp + s) * dp * 2);
-      const float4* qv = reinterpret_cast<const float4*>(sqp + hl * dp);
-      float acc = 0.f;
-#pragma unroll 1
-      for (int c = 0; c < lpr; ++c) {
-        const uint4 v = row[c];
-        const float4 q0 = qv[2 * c], q1 = qv[2 * c + 1];
-        acc = fmaf(__uint_as_float(v.x << 16), q0.x, acc); acc = fmaf(__uint_as_float(v.x & 0xffff0000u), q0.y, acc);
-        acc = fmaf(__uint_as_float(v.y << 16), q0.z, acc); acc = fmaf(__uint_as_float(v.y & 0xffff0000u), q0.w, acc);
-        acc = fmaf(__uint_as_float(v.z << 16), q1.x, acc); acc = fmaf(__uint_as_float(v.z & 0xffff0000u), q1.y, acc);
-        acc = fmaf(__uint_as_float(v.w << 16), q1.z, acc); acc = fmaf(__uint_as_float(v.w & 0xffff0000u), q1.w, acc);
-      }
-      const float x = fmaf(acc, inv_sqrt_dp, lnl);            // Eq. 5, pre-sigmoid logit
-      const float a = 1.f / (1.f + __expf(-x));
-      const int h = g * G + hl;
-      if (P.logits_out) P.logits_out[(size_t)h * P.m_tot + I.span0 + I.a + s] = x;
-      if (P.alpha_out) P.alpha_out[(size_t)h * P.m_tot + I.span0 + I.a + s] = a;
-      if (P.tau != nullptr && a > P.tau[h]) elig = true;       // Eq. 9
-      X = fmaxf(X, x);
-    }
-    gkeys[I.a + s] = elig ? order_key(X) : 0u;
-  }
-  mark(tm, 2, lane);
-  signal_ctr(grp_ctr(P, bg, C_ROUTE), lane);
-}
-
-// ---------------------------------------------------------------------------------------------------
-// a3 + a4 by a TEAM: the CTA's latency warps (the even warps, TS = 32 * ceil(nw / 2) threads) meet on named
-// barrier 1 once the latency queue is exhausted and run selection and residency plan of the groups
-// bg = blockIdx.x, + gridDim.x, ... together -- a single warp runs this serial chain at ~200 instructions
-// per microsecond, and every expanded span of the group waits for it.  Tables live in the region of warp 0.
-// ---------------------------------------------------------------------------------------------------
-struct Team { int tt, ts, lane, tw, ntw; int* scratch; };
+struct Team { int tt, ts, lane, tw, ntw; int* scratch; uint8_t* tab; uint8_t* stage; uint64_t* bars; uint32_t ph[2]; };
 
 __device__ __forceinline__ void team_bar(const Team& T) { asm volatile("bar.sync 1, %0;" ::"r"(T.ts) : "memory"); }
 
@@ -298,18 +159,42 @@ __device__ __forceinline__ int team_excl_scan(const Team& T, int v, int* total) 
   return base + ex;
 }
 
-// descending bitonic sort of n (power of two) 64-bit keys in shared memory by the team
-__device__ __forceinline__ void bitonic_sort_desc_team(const Team& T, unsigned long long* keys, int n) {
-  for (int size = 2; size <= n; size <<= 1) {
-    for (int stride = size >> 1; stride > 0; stride >>= 1) {
-      for (int i = T.tt; i < (n >> 1); i += T.ts) {
-        const int lo = ((i & ~(stride - 1)) << 1) | (i & (stride - 1));
-        const int hi = lo | stride;
-        const bool desc = ((lo & size) == 0);
-        const unsigned long long a = keys[lo], c = keys[hi];
-        if ((a < c) == desc) { keys[lo] = c; keys[hi] = a; }
-      }
-      team_bar(T);
+// ---------------------------------------------------------------------------------------------------
+// a1 (Eq. 4): q'_h = W_h q_h for one query head on the tensor cores: the rows of W_h are the M dimension
+// (16 per tile), the group's queries are the 8 columns, column hl of the result is q'_hl -> shared memory.
+// ---------------------------------------------------------------------------------------------------
+template <int G>
+__device__ __forceinline__ void qproj_load(const FusedParams& P, int b, int g, int hl, int j0, int lane,
+                                           uint32_t (&qf)[4][4], uint4 (&w)[2][2][4]) {
+  const int dp = P.dp, gid = lane >> 2, t4 = lane & 3;
+  if (j0 == 0) load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
+  const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)(g * G + hl) * dp * (kD * 2) + t4 * 16;
+#pragma unroll
+  for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+      const int row = j0 + 16 * mt + 8 * hf + gid;
+#pragma unroll
+      for (int jj = 0; jj < 4; ++jj)
+        w[mt][hf][jj] = row < dp ? ldg16(Wh + (size_t)row * (kD * 2) + jj * 64) : make_uint4(0u, 0u, 0u, 0u);
+    }
+}
+template <int G>
+__device__ __forceinline__ void qproj_mma(const FusedParams& P, int hl, int j0, int lane, const uint32_t (&qf)[4][4],
+                                          const uint4 (&w)[2][2][4], float* dst) {
+  const int dp = P.dp, gid = lane >> 2, t4 = lane & 3;
+#pragma unroll
+  for (int mt = 0; mt < 2; ++mt) {
+    float c[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {
+      mma16816_full(c, w[mt][0][jj].x, w[mt][1][jj].x, w[mt][0][jj].y, w[mt][1][jj].y, qf[jj][0], qf[jj][1]);
+      mma16816_full(c, w[mt][0][jj].z, w[mt][1][jj].z, w[mt][0][jj].w, w[mt][1][jj].w, qf[jj][2], qf[jj][3]);
+    }
+    if (t4 == (hl >> 1)) {                                     // this lane holds column hl of the tile
+      const int r = j0 + 16 * mt + gid;
+      if (r < dp) dst[r] = (hl & 1) ? c[1] : c[0];
+      if (r + 8 < dp) dst[r + 8] = (hl & 1) ? c[3] : c[2];
     }
   }
 }
@@ -325,6 +210,8 @@ __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, in
     const int len = (int)(meta >> 16);
     d.len_rr = meta;
     d.bytes = (uint32_t)blob_dims(2, len, rr & 0xff, (rr >> 8) & 0xff).bytes;
+    // hits: the cache slot; misses: the device alias of the pinned-host store (the ZOOM item copies the blob into
+    // its slot first when it has one)
     const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
                                             : P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
     d.src = (unsigned long long)src;
@@ -337,45 +224,203 @@ __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, in
 struct PlanTables {
   int32_t* sh_ids; int16_t* way_of; int32_t* sh_tag; uint32_t* sh_stamp; int32_t* sh_victim; uint32_t* sh_mask;
   uint32_t* meta;      // [m] |S| << 16 | rank_k | rank_v << 8 of every span of the group
+  float* lnl;          // [m] ln|S|
 };
-__device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t* region) {
+__device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t* tab) {
   PlanTables t;
-  t.sh_ids = reinterpret_cast<int32_t*>(region + P.sm_ids);
-  t.way_of = reinterpret_cast<int16_t*>(region + P.sm_wayof);
-  t.sh_tag = reinterpret_cast<int32_t*>(region + P.sm_tags);
+  t.sh_ids = reinterpret_cast<int32_t*>(tab + P.sm_ids);
+  t.way_of = reinterpret_cast<int16_t*>(tab + P.sm_wayof);
+  t.sh_tag = reinterpret_cast<int32_t*>(tab + P.sm_tags);
   t.sh_stamp = reinterpret_cast<uint32_t*>(t.sh_tag + P.ways);
   t.sh_victim = reinterpret_cast<int32_t*>(t.sh_stamp + P.ways);
-  t.sh_mask = reinterpret_cast<uint32_t*>(region + P.sm_mask);
-  t.meta = reinterpret_cast<uint32_t*>(region + P.sm_meta);
+  t.sh_mask = reinterpret_cast<uint32_t*>(tab + P.sm_mask);
+  t.meta = reinterpret_cast<uint32_t*>(tab + P.sm_meta);
+  t.lnl = reinterpret_cast<float*>(tab + P.sm_lnl);
   return t;
 }
 
-// first half of the plan: needs nothing from this step's routing, runs while the ROUTE items are in flight
-__device__ __forceinline__ void plan_init_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
+// Tables that need nothing from this step's routing -> shared memory by 4-byte cp.async copies, all in flight at
+// once (no register round trip): span meta (the directory word carries |S| and both ranks), ln|S|, cache tags and
+// stamps.  The caller commits / waits and runs a team barrier; _scatter then inverts the tags into way_of.
+__device__ __forceinline__ void r_select_end(unsigned long long*) {}
+__device__ __forceinline__ void plan_init_fill(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
                                                int m) {
   const int g = bg % P.Hkv;
-  for (int s0 = 0; s0 < m; s0 += 8 * T.ts) {                   // 16 loads in flight per thread
-    int len[8], rr[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      const int s = min(s0 + u * T.ts + T.tt, m - 1);
-      len[u] = P.cv.span_len[span0 + s];
-      rr[u] = P.lv.dir_rank[(size_t)g * P.spans_cap + span0 + s];
+  const int32_t* dirw = P.lv.dir_rank + (size_t)g * P.spans_cap + span0;
+  const float* lnl = P.cv.ln_len + span0;
+#pragma unroll 1
+  for (int s = T.tt; s < m; s += T.ts) { cp_async4(t.meta + s, dirw + s); cp_async4(t.lnl + s, lnl + s); t.way_of[s] = (int16_t)-1; }
+  if (P.mode & FM_ATTN) {
+    const int32_t* tags = P.lv.tags + (size_t)bg * P.ways;
+    const uint32_t* stamps = P.lv.stamps + (size_t)bg * P.ways;
+#pragma unroll 1
+    for (int w = T.tt; w < P.ways; w += T.ts) { cp_async4(t.sh_tag + w, tags + w); cp_async4(t.sh_stamp + w, stamps + w); t.sh_victim[w] = -1; }
+  }
+  cp_async_commit();
+  for (int w = T.tt; w < P.mask_words; w += T.ts) t.sh_mask[w] = 0u;
+}
+__device__ __forceinline__ void plan_init_scatter(const FusedParams& P, const Team& T, const PlanTables& t, int m) {
+  for (int w = T.tt; w < P.ways; w += T.ts) { const int tg = t.sh_tag[w]; if (tg >= 0 && tg < m) t.way_of[tg] = (int16_t)w; }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a1 + a2 + GQA reduce of a3 (Eq. 4, 5, 9) by the team: q' -> shared memory; the G x m rows of the routing
+// table of (b, g) stream through the team warps' staging buffers in blocks of P.route_spans spans (cp.async,
+// P.route_bufs deep), ordered 32-bit keys -> shared memory.  Fast path (d' = 32, no threshold, no score
+// outputs): per head, 16 staged rows are the M dimension of mma tiles, q' (split into bf16 hi + lo, ~16
+// bits) the columns.  General path: compact scalar loops.
+// ---------------------------------------------------------------------------------------------------
+template <int G>
+__device__ __forceinline__ void route_team(const FusedParams& P, Team& T, int bg, uint32_t* keys,
+                                           float* sqp, const PlanTables& pt, int* span0_out, int* m_out,
+                                           unsigned long long* tm) {
+  const int b = bg / P.Hkv, g = bg % P.Hkv, dp = P.dp, lpr = dp >> 3, lane = T.lane;
+  // the query and W of this warp's head go first: they need nothing but the group index
+  uint32_t qf[4][4];
+  uint4 wq[2][2][4];
+  const int my_hl = T.tw;
+  if (my_hl < G) qproj_load<G>(P, b, g, my_hl, 0, lane, qf, wq);
+  const int2 gi = __ldg(P.grp + bg);                             // first span and span count of the group's sequence
+  const int span0 = gi.x, m = gi.y;
+  *span0_out = span0; *m_out = m;
+  const int gid = lane >> 2, t4 = lane & 3;
+  const int nsp_blk = P.route_spans, nbuf = P.route_bufs;
+  const int nblk = (m + nsp_blk - 1) / nsp_blk;
+  const uint8_t* route = (const uint8_t*)P.lv.route;
+  const uint32_t buf_bytes = (uint32_t)nsp_blk * G * dp * 2;
+  // one 1-D bulk copy per head: the rows of a block are contiguous in the routing table and in the staging buffer
+  auto issue = [&](int blk, int buf) {
+    __syncwarp();                                              // every lane is done reading this buffer
+    if (lane == 0) {
+      const int s_lo = blk * nsp_blk, nsp = min(m, s_lo + nsp_blk) - s_lo;
+      uint8_t* dst = T.stage + (size_t)buf * buf_bytes;
+      const uint32_t hb = (uint32_t)nsp * dp * 2;
+      mbar_arrive_expect_tx(&T.bars[buf], hb * G);
+#pragma unroll 1
+      for (int hl = 0; hl < G; ++hl)
+        bulk_g2s(dst + (size_t)hl * hb, route + ((size_t)(g * G + hl) * P.route_head_stride + (size_t)(span0 + s_lo) * dp) * 2,
+                 hb, &T.bars[buf]);
     }
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      const int s = s0 + u * T.ts + T.tt;
-      if (s < m) t.meta[s] = ((uint32_t)len[u] << 16) | (uint32_t)(rr[u] & 0xffff);
+  };
+  int blk = T.tw, buf = 0;
+  if (blk < nblk) issue(blk, 0);
+  if (nbuf == 2 && blk + T.ntw < nblk) issue(blk + T.ntw, 1);
+  plan_init_fill(P, T, pt, bg, span0, m);                       // independent of the routing: its loads overlap
+  int* sel = T.scratch + 16;                                     // [2..4] eligible keys / min key / max key
+  if (T.tt == 0) { sel[2] = 0; sel[3] = -1; sel[4] = 0; sel[5] = 0; sel[6] = 0; }
+  {
+    uint32_t* hist = reinterpret_cast<uint32_t*>(T.tab + P.sm_hist);     // one histogram per radix pass of the select
+    for (int i = T.tt; i < 4 * 256; i += T.ts) hist[i] = 0u;
+  }
+  if (my_hl < G) {
+    qproj_mma<G>(P, my_hl, 0, lane, qf, wq, sqp + my_hl * dp);
+    for (int j0 = 32; j0 < dp; j0 += 32) {                       // d' = 64: the second half of W_h
+      qproj_load<G>(P, b, g, my_hl, j0, lane, qf, wq);
+      qproj_mma<G>(P, my_hl, j0, lane, qf, wq, sqp + my_hl * dp);
     }
   }
-  const int32_t* tags = P.lv.tags + (size_t)bg * P.ways;
-  const uint32_t* stamps = P.lv.stamps + (size_t)bg * P.ways;
-  for (int w = T.tt; w < P.mask_words; w += T.ts) t.sh_mask[w] = 0u;
-  for (int s = T.tt; s < m; s += T.ts) t.way_of[s] = (int16_t)-1;
-  for (int w = T.tt; w < P.ways; w += T.ts) { t.sh_tag[w] = tags[w]; t.sh_stamp[w] = stamps[w]; t.sh_victim[w] = -1; }
-  team_bar(T);
-  for (int w = T.tt; w < P.ways; w += T.ts) { const int tg = t.sh_tag[w]; if (tg >= 0 && tg < m) t.way_of[tg] = (int16_t)w; }
-  team_bar(T);
+  for (int hl = my_hl + T.ntw; hl < G; hl += T.ntw)              // (teams with fewer warps than heads)
+    for (int j0 = 0; j0 < dp; j0 += 32) {
+      qproj_load<G>(P, b, g, hl, j0, lane, qf, wq);
+      qproj_mma<G>(P, hl, j0, lane, qf, wq, sqp + hl * dp);
+    }
+  cp_async_wait<0>();
+  team_bar(T);                                                   // q' of the group and the plan tables are in shared memory
+  if (P.mode & FM_ATTN) plan_init_scatter(P, T, pt, m);
+  int ne = 0;
+  uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+  const float inv_sqrt_dp = rsqrtf((float)dp);
+  const bool fast = dp == 32 && P.tau == nullptr && P.logits_out == nullptr && P.alpha_out == nullptr;
+  uint32_t bh[4] = {0u, 0u, 0u, 0u}, bl[4] = {0u, 0u, 0u, 0u};
+  if (fast && gid < G) {
+    const float4 v0 = *reinterpret_cast<const float4*>(sqp + gid * 32 + 8 * t4);
+    const float4 v1 = *reinterpret_cast<const float4*>(sqp + gid * 32 + 8 * t4 + 4);
+    split_bf16(v0.x * inv_sqrt_dp, v0.y * inv_sqrt_dp, bh[0], bl[0]);
+    split_bf16(v0.z * inv_sqrt_dp, v0.w * inv_sqrt_dp, bh[1], bl[1]);
+    split_bf16(v1.x * inv_sqrt_dp, v1.y * inv_sqrt_dp, bh[2], bl[2]);
+    split_bf16(v1.z * inv_sqrt_dp, v1.w * inv_sqrt_dp, bh[3], bl[3]);
+  }
+  for (; blk < nblk; blk += T.ntw) {
+    mbar_wait(&T.bars[buf], T.ph[buf]);
+    T.ph[buf] ^= 1u;
+    const int s_lo = blk * nsp_blk, nsp = min(m, s_lo + nsp_blk) - s_lo;
+    const uint8_t* src = T.stage + (size_t)buf * buf_bytes;
+    if (fast) {
+#pragma unroll 1
+      for (int s0 = 0; s0 < nsp; s0 += 16) {
+        float Xa = -INFINITY, Xb = -INFINITY;                      // spans s0 + gid and s0 + gid + 8
+#pragma unroll
+        for (int hl = 0; hl < G; ++hl) {
+          const uint8_t* ra = src + ((size_t)hl * nsp + s0 + gid) * 64 + t4 * 16;
+          const uint4 a = *reinterpret_cast<const uint4*>(ra), c8 = *reinterpret_cast<const uint4*>(ra + 8 * 64);
+          float c[4] = {0.f, 0.f, 0.f, 0.f};
+          mma16816_full(c, a.x, c8.x, a.y, c8.y, bh[0], bh[1]);
+          mma16816_full(c, a.z, c8.z, a.w, c8.w, bh[2], bh[3]);
+          mma16816_full(c, a.x, c8.x, a.y, c8.y, bl[0], bl[1]);
+          mma16816_full(c, a.z, c8.z, a.w, c8.w, bl[2], bl[3]);
+          if (t4 == (hl >> 1)) {                                   // this lane holds column hl
+            Xa = fmaxf(Xa, (hl & 1) ? c[1] : c[0]);
+            Xb = fmaxf(Xb, (hl & 1) ? c[3] : c[2]);
+          }
+        }
+        Xa = quad_max(Xa); Xb = quad_max(Xb);
+        const int s = s0 + gid + 8 * (t4 & 1);
+        if (t4 < 2 && s < nsp) {
+          const uint32_t k = order_key(((t4 & 1) ? Xb : Xa) + pt.lnl[s_lo + s]);
+          keys[s_lo + s] = k;
+          ++ne; kmin = min(kmin, k); kmax = max(kmax, k);
+        }
+      }
+    } else {
+      for (int s = lane; s < nsp; s += 32) {
+        const float lnl = pt.lnl[s_lo + s];
+        float X = -INFINITY;
+        bool elig = (P.tau == nullptr);
+#pragma unroll 1
+        for (int hl = 0; hl < G; ++hl) {
+          const uint4* row = reinterpret_cast<const uint4*>(src + ((size_t)hl * nsp + s) * dp * 2);
+          const float4* qv = reinterpret_cast<const float4*>(sqp + hl * dp);
+          float acc = 0.f;
+#pragma unroll 1
+          for (int c = 0; c < lpr; ++c) {
+            const uint4 v = row[c];
+            const float4 q0 = qv[2 * c], q1 = qv[2 * c + 1];
+            acc = fmaf(__uint_as_float(v.x << 16), q0.x, acc); acc = fmaf(__uint_as_float(v.x & 0xffff0000u), q0.y, acc);
+            acc = fmaf(__uint_as_float(v.y << 16), q0.z, acc); acc = fmaf(__uint_as_float(v.y & 0xffff0000u), q0.w, acc);
+            acc = fmaf(__uint_as_float(v.z << 16), q1.x, acc); acc = fmaf(__uint_as_float(v.z & 0xffff0000u), q1.y, acc);
+            acc = fmaf(__uint_as_float(v.w << 16), q1.z, acc); acc = fmaf(__uint_as_float(v.w & 0xffff0000u), q1.w, acc);
+          }
+          const float x = fmaf(acc, inv_sqrt_dp, lnl);            // Eq. 5, pre-sigmoid logit
+          const float a = 1.f / (1.f + __expf(-x));
+          const int h = g * G + hl;
+          if (P.logits_out) P.logits_out[(size_t)h * P.m_tot + span0 + s_lo + s] = x;
+          if (P.alpha_out) P.alpha_out[(size_t)h * P.m_tot + span0 + s_lo + s] = a;
+          if (P.tau != nullptr && a > P.tau[h]) elig = true;       // Eq. 9
+          X = fmaxf(X, x);
+        }
+        const uint32_t k = elig ? order_key(X) : 0u;
+        keys[s_lo + s] = k;
+        if (k != 0u) { ++ne; kmin = min(kmin, k); kmax = max(kmax, k); }
+      }
+    }
+    const int nb = blk + nbuf * T.ntw;                           // the block that reuses this buffer
+    if (nb < nblk) issue(nb, buf);
+    if (nbuf == 2) buf ^= 1;
+  }
+  // eligible keys, smallest and largest key of the group (what the radix select starts from)
+  ne = warp_sum_i(ne);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+    kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+  }
+  if (lane == 0 && ne > 0) {
+    atomicAdd(&sel[2], ne);
+    atomicMin(reinterpret_cast<unsigned int*>(&sel[3]), kmin);
+    atomicMax(reinterpret_cast<unsigned int*>(&sel[4]), kmax);
+  }
+  team_bar(T);                                                   // the keys of the group are complete
+  mark(tm, 0, T.tt);
 }
 
 // a4: residency plan of (b, g).  The device factor cache of a (layer, sequence, kv head) is `ways` slots with
@@ -383,11 +428,12 @@ __device__ __forceinline__ void plan_init_team(const FusedParams& P, const Team&
 // set: resident ones are hits, the others are demand misses and take the least-recently-used slots not
 // needed by this step.  Entries n_zoom .. n_cand-1 are prefetch candidates (the next-best spans by routing
 // score): the non-resident ones get a slot too and are copied by the side-stream prefetch kernel after
-// this layer's kernel.  Also: zoom bit-mask for the coarse items (an expanded span's coarse entry is
+// this layer's kernel.  Also: zoom bit-mask for the COARSE items (an expanded span's coarse entry is
 // replaced by its tokens), de-duplication of caller-supplied ids, one descriptor per
 // expanded span for the ZOOM items, statistics.
 __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
-                                          int m, int n_zoom, int n_cand, bool dedupe, uint32_t epoch) {
+                                          int m, int n_zoom, int n_cand, bool dedupe, uint32_t epoch,
+                                          unsigned long long* tm = nullptr) {
   const int g = bg % P.Hkv, ways = P.ways;
   int32_t* tags = P.lv.tags + (size_t)bg * ways;
   uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
@@ -395,8 +441,8 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   int32_t* item_span = P.lv.item_span + (size_t)bg * P.kc;
   ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
   const uint32_t cur = epoch;
-  int n_hit = 0, n_miss = 0, n_pf = 0;
-  unsigned long long bytes_algo = 0, bytes_h2d = 0;
+  int n_hit = 0, n_miss = 0, n_pf = 0, n_pf_slot = 0;
+  unsigned long long bytes_algo = 0, bytes_demand = 0, bytes_pf = 0;
   // pass 1: validate / de-duplicate, zoom mask, residency lookup
   for (int j = T.tt; j < n_cand; j += T.ts) {
     int id = t.sh_ids[j];
@@ -415,11 +461,11 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       meta = t.meta[id];
       const int rk = meta & 0xff, rv = (meta >> 8) & 0xff;
       const int len = (int)(meta >> 16);
-      const unsigned long long bb = blob_dims(2, len, rk, rv).bytes;
       if (zoom) {
         bytes_algo += (unsigned long long)(rk + rv) * (len + kD) * 2 + 4ull * (rk + rv);
-        if (way >= 0) ++n_hit; else { ++n_miss; bytes_h2d += bb; }
-      } else if (way < 0) { ++n_pf; bytes_h2d += bb; }
+        if (way >= 0) ++n_hit;
+        else { ++n_miss; bytes_demand += blob_dims(2, len, rk, rv).bytes; }
+      } else if (way < 0) ++n_pf;
     }
     t.sh_ids[j] = id;
     item_span[j] = id;
@@ -430,8 +476,14 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   }
   for (int j = n_zoom + T.tt; j < min(P.k_cap, m); j += T.ts) write_zdesc(P, zd + j, bg, g, span0, -1, 0u, 0u, epoch);
   int n_need;
-  team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1)
+  team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1 to the team)
   n_need = min(n_need, ways);
+  // the zoom mask is all the COARSE items wait for: published before the misses are given slots, as
+  // self-validating (bits, step stamp) pairs -- 8-byte stores that the COARSE items poll, no flag, no fence
+  uint2* gmask = P.zmask2 + (size_t)bg * P.mask_words;
+  for (int w = T.tt; w < P.mask_words; w += T.ts) gmask[w] = make_uint2(t.sh_mask[w], epoch);
+  if (T.tt == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
+  mark(tm, 3, T.tt);
   // victims: the n_need oldest ways not used by this step (ties to the lower way), by repeated extraction
   // of the minimum (stamp, way) -- only as many as this step has misses
   if (T.tw == 0) {
@@ -463,6 +515,11 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       if (way >= 0) {
         t.sh_tag[way] = id;
         it = (uint32_t)way | 0x80000000u;
+        if (j >= n_zoom) {                                     // a prefetch candidate that will be copied
+          const uint32_t meta = t.meta[id];
+          ++n_pf_slot;
+          bytes_pf += blob_dims(2, (int)(meta >> 16), meta & 0xff, (meta >> 8) & 0xff).bytes;
+        }
       } else {
         it = 0xC0000000u;                                      // no free slot: fetch, do not keep
       }
@@ -473,17 +530,13 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
-  uint32_t* gmask = P.lv.zoom_mask + (size_t)bg * P.mask_words;
-  for (int w = T.tt; w < P.mask_words; w += T.ts) gmask[w] = t.sh_mask[w];
-  if (T.tt == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
-  team_bar(T);                                                 // every thread's global writes precede the release
-  if (T.tt == 0) red_add_release(grp_ctr(P, bg, C_PLAN), 1);
   // statistics (off the critical path)
-  n_hit = warp_sum_i(n_hit); n_miss = warp_sum_i(n_miss); n_pf = warp_sum_i(n_pf);
+  n_hit = warp_sum_i(n_hit); n_miss = warp_sum_i(n_miss); n_pf_slot = warp_sum_i(n_pf_slot);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
-    bytes_h2d += __shfl_xor_sync(0xffffffffu, bytes_h2d, o);
+    bytes_demand += __shfl_xor_sync(0xffffffffu, bytes_demand, o);
+    bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
   }
   if (T.lane == 0) {
     if (n_hit) atomicAdd(&P.stats[ST_HITS], (unsigned long long)n_hit);
@@ -493,79 +546,24 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       atomicAdd(&P.stats[ST_SKIPPED], (unsigned long long)(n_hit + n_miss));
     }
     if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
-    if (bytes_h2d) atomicAdd(&P.stats[ST_H2D], bytes_h2d);
-    if (n_pf) atomicAdd(&P.stats[ST_PREFETCHED], (unsigned long long)n_pf);
+    if (bytes_demand) atomicAdd(&P.stats[ST_H2D], bytes_demand);
+    if (bytes_pf) atomicAdd(&P.stats[ST_PF_BYTES], bytes_pf);
+    if (n_pf_slot) atomicAdd(&P.stats[ST_PREFETCHED], (unsigned long long)n_pf_slot);
   }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a3 (Eq. 9, cap L123): top-n_cand of the group's m keys.  A radix select (8 bits per pass, shared-memory
-// histogram, starting at the highest bit in which the eligible keys differ) finds the n_cand-th largest
-// key T; keys > T are taken, keys == T are taken in increasing span id until the count is met (ties to the
-// lower id); the <= kc winners are then sorted by (key descending, id ascending).
+// a3 (Eq. 9, cap L123): top-n_cand of the group's m keys (shared memory).  A radix select (8 bits per pass,
+// shared-memory histograms, starting at the highest bit in which the eligible keys differ) finds the
+// n_cand-th largest key T; keys > T are taken, keys == T are taken in increasing span id until the count is
+// met (ties to the lower id); the winners are then ranked by (key descending, id ascending).
+// Returns cnt (zoom set) and n_cand (zoom set + prefetch candidates); ids in t.sh_ids.
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void select_team(const FusedParams& P, const Team& T, uint8_t* region, int bg, uint32_t epoch,
-                                            unsigned long long* tm) {
-  const int b = bg / P.Hkv;
-  const int span0 = P.cv.seq_span_off[b];
-  const int m = P.cv.seq_span_off[b + 1] - span0;
-  const PlanTables t = plan_tables(P, region);
-  if (P.mode & FM_ATTN) plan_init_team(P, T, t, bg, span0, m);
-  if (!(P.mode & FM_ROUTE)) {
-    // caller-supplied zoom set (sekv_decode_attn)
-    int cnt = 0;
-    if (P.ids != nullptr && P.count != nullptr) cnt = max(0, min(P.count[bg], P.k_cap));
-    const int32_t* src = P.ids + (size_t)bg * max(P.k_cap, 1);
-    for (int j = T.tt; j < cnt; j += T.ts) t.sh_ids[j] = src[j];
-    team_bar(T);
-    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch);
-    return;
-  }
-  uint32_t* keys = reinterpret_cast<uint32_t*>(region);
-  uint32_t* hist = reinterpret_cast<uint32_t*>(region + P.sm_hist);
-  unsigned long long* cand = reinterpret_cast<unsigned long long*>(region + P.sm_cand);
-  int* sel = T.scratch + 8;                // [0] digit, [1] keys above it, [2..4] ne / kmin / kmax, [5] keys == T, [6] slot
-  for (int i = T.tt; i < 4 * 256; i += T.ts) hist[i] = 0u;     // one histogram per radix pass, zeroed while waiting
-  const uint32_t* gkeys = P.keys + (size_t)bg * P.keys_stride;
-  const int n_route = (m + P.route_spans - 1) / P.route_spans;
-  if (T.tt == 0) {
-    const int32_t* c = grp_ctr(P, bg, C_ROUTE);
-    int v;
-    for (;;) {
-      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
-      if (v >= n_route) break;
-      __nanosleep(64);
-    }
-    (void)ld_acquire(reinterpret_cast<const uint32_t*>(c));
-    sel[2] = 0; sel[3] = -1; sel[4] = 0; sel[5] = 0; sel[6] = 0;
-    mark(tm, 0, 0);
-  }
-  team_bar(T);
-  for (int i = T.tt; i < (m + 3) / 4; i += T.ts) cp_async16(keys + 4 * i, gkeys + 4 * i);   // all in flight at once
-  cp_async_commit();
-  cp_async_wait<0>();
-  team_bar(T);
-  mark(tm, 1, T.tt);
-  {
-    int ne = 0;
-    uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-    for (int i = T.tt; i < m; i += T.ts) {
-      const uint32_t k = keys[i];
-      if (k != 0u) { ++ne; kmin = min(kmin, k); kmax = max(kmax, k); }
-    }
-    ne = warp_sum_i(ne);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
-      kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
-    }
-    if (T.lane == 0) {
-      atomicAdd(&sel[2], ne);
-      atomicMin(reinterpret_cast<unsigned int*>(&sel[3]), kmin);
-      atomicMax(reinterpret_cast<unsigned int*>(&sel[4]), kmax);
-    }
-  }
-  team_bar(T);
+__device__ __forceinline__ void select_team(const FusedParams& P, const Team& T, const PlanTables& t, const uint32_t* keys,
+                                            int m, int* cnt_out, int* ncand_out, unsigned long long* tm) {
+  uint32_t* hist = reinterpret_cast<uint32_t*>(T.tab + P.sm_hist);
+  unsigned long long* cand = reinterpret_cast<unsigned long long*>(T.tab + P.sm_cand);
+  int* sel = T.scratch + 16;     // [0] digit, [1] keys above it, [2..4] ne / kmin / kmax, [5] keys == T, [6] slot
   const int n_elig = sel[2];
   const uint32_t kmin = (uint32_t)sel[3], kmax = (uint32_t)sel[4];
   int cnt = P.k < 0 ? n_elig : min(P.k, n_elig);
@@ -574,9 +572,8 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
   if (P.k >= 0 && (P.mode & FM_ATTN)) n_cand = min(min(cnt + P.prefetch, n_elig), P.kc);
   uint32_t Tk = 0u;           // threshold key
   int need = 0;               // keys == Tk to take
-  if (n_cand == 0) {
-    Tk = 0xFFFFFFFFu;
-  } else if (n_cand < n_elig) {
+  const bool partial = n_cand != 0 && n_cand < n_elig;
+  if (partial) {
     // the eligible keys agree on every bit above the highest bit in which kmin and kmax differ: the passes
     // start there (float keys of one binade share 9 bits: a pass over them would pile every key -- and
     // every shared-memory atomic -- into one bin)
@@ -586,6 +583,7 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
     uint32_t prefix = kmax & maskb;
     need = n_cand;
     uint32_t* hp = hist;
+#pragma unroll 1
     for (int shift = top; shift >= 0; shift = (shift >= 8 ? shift - 8 : (shift > 0 ? 0 : -1)), hp += 256) {
       for (int i = T.tt; i < m; i += T.ts) {
         const uint32_t k = keys[i];
@@ -607,86 +605,134 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
       need -= sel[1];
       prefix |= (uint32_t)sel[0] << shift;
       maskb |= 255u << shift;
+      if (sel[5] == need) break;        // every key of this bin is taken: the lower bits need not be resolved
     }
-    Tk = prefix;
+    Tk = prefix;                        // (after an early exit: the smallest possible key of the bin)
   }
-  mark(tm, 2, T.tt);
-  const bool cut_ties = (n_cand != 0 && n_cand < n_elig) && sel[5] != need;   // more keys == T than are taken
-  if (!cut_ties) {
-    // every key >= T is taken: append in any order (the sort below fixes the order)
-    const uint32_t lo_key = (n_cand != 0 && n_cand < n_elig) ? Tk : (n_cand == 0 ? 0xFFFFFFFFu : 1u);
-    if (n_cand != 0)
-      for (int i = T.tt; i < m; i += T.ts) {
-        const uint32_t k = keys[i];
-        if (k >= lo_key) {
-          const int pos = atomicAdd(&sel[6], 1);
-          if (pos < P.kc) cand[pos] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
-        }
+  mark(tm, 1, T.tt);
+  // winners: every eligible key (n_cand == n_elig), or the keys > T plus `need` keys == T.  When more keys
+  // equal T than are taken, those are taken in increasing span id (ties to the lower id): the rank of a tied
+  // key among its equals is counted directly (ties at the cut are rare and few).
+  const bool cut_ties = partial && sel[5] != need;
+  if (n_cand != 0)
+    for (int i = T.tt; i < m; i += T.ts) {
+      const uint32_t k = keys[i];
+      bool take = partial ? (k > Tk || (k == Tk && !cut_ties)) : (k != 0u);
+      if (k == 0u) take = false;
+      if (partial && cut_ties && k == Tk) {
+        int before = 0;
+        for (int j = 0; j < i; ++j) before += (keys[j] == Tk);
+        take = before < need;
       }
-    team_bar(T);
-  } else {
-  // ordered compaction: each thread owns a contiguous block of span ids
-  const int per = (m + T.ts - 1) / T.ts;
-  const int lo = min(m, T.tt * per), hi = min(m, lo + per);
-  int gt = 0, eq = 0;
-  for (int i = lo; i < hi; ++i) { const uint32_t k = keys[i]; gt += (k > Tk); eq += (k == Tk); }
-  int dummy;
-  const int eq_before = team_excl_scan(T, eq, &dummy);
-  const int take_eq = (Tk == 0u) ? 0 : max(0, min(eq, need - eq_before));
-  int pos = team_excl_scan(T, gt + take_eq, &dummy);
-  int taken = 0;
-  for (int i = lo; i < hi; ++i) {
-    const uint32_t k = keys[i];
-    bool s = k > Tk;
-    if (k == Tk && taken < take_eq) { s = true; ++taken; }
-    if (s && pos < P.kc) cand[pos++] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
-  }
-  team_bar(T);
-  }
-  if (n_cand <= T.ts) {
-    if (T.tt < n_cand) {
-      const unsigned long long mine = cand[T.tt];
-      int r = 0;
-      for (int i = 0; i < n_cand; ++i) r += (cand[i] > mine);
-      t.sh_ids[r] = (int32_t)(0xFFFFFFFFu - (uint32_t)(mine & 0xFFFFFFFFull));
+      if (take) {
+        const int pos = atomicAdd(&sel[6], 1);
+        if (pos < P.kc) cand[pos] = ((unsigned long long)k << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)i);
+      }
     }
-  } else {
-    int n2 = 64;
-    while (n2 < n_cand) n2 <<= 1;
-    for (int j = n_cand + T.tt; j < n2; j += T.ts) cand[j] = 0ull;
-    team_bar(T);
-    bitonic_sort_desc_team(T, cand, n2);
-    for (int j = T.tt; j < n_cand; j += T.ts) t.sh_ids[j] = (int32_t)(0xFFFFFFFFu - (uint32_t)(cand[j] & 0xFFFFFFFFull));
+  team_bar(T);
+  // rank by (key descending, id ascending): the composite 64-bit values are distinct
+  for (int j = T.tt; j < n_cand; j += T.ts) {
+    const unsigned long long mine = cand[j];
+    int r = 0;
+    for (int i = 0; i < n_cand; ++i) r += (cand[i] > mine);
+    t.sh_ids[r] = (int32_t)(0xFFFFFFFFu - (uint32_t)(mine & 0xFFFFFFFFull));
   }
   team_bar(T);
-  mark(tm, 3, T.tt);
-  int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
-  for (int j = T.tt; j < P.k_cap; j += T.ts) my_ids[j] = j < cnt ? t.sh_ids[j] : -1;
-  if (T.tt == 0) P.count[bg] = cnt;
-  if (P.mode & FM_ATTN) plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch);
+  mark(tm, 2, T.tt);
+  *cnt_out = cnt; *ncand_out = n_cand;
 }
 
-// one partial record (m2, l, pad, pad, o[128]) per head; lane (gid, t4) holds head gid's (m, l) and the
-// accumulators listed by the callers
+// ---------------------------------------------------------------------------------------------------
+// The whole chain a1-a4 of group bg by the team.
+// ---------------------------------------------------------------------------------------------------
+template <int G>
+__device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int bg, uint32_t epoch,
+                                            unsigned long long* tm) {
+  const PlanTables t = plan_tables(P, T.tab);
+  uint32_t* keys = reinterpret_cast<uint32_t*>(T.tab + P.sm_keys);
+  float* sqp = reinterpret_cast<float*>(T.tab + P.sm_qp);
+  int span0, m;
+  if (P.mode & FM_ROUTE) {
+    route_team<G>(P, T, bg, keys, sqp, t, &span0, &m, tm);
+    int cnt, n_cand;
+    select_team(P, T, t, keys, m, &cnt, &n_cand, tm);
+    int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
+    for (int j = T.tt; j < P.k_cap; j += T.ts) my_ids[j] = j < cnt ? t.sh_ids[j] : -1;
+    if (T.tt == 0) P.count[bg] = cnt;
+    if (P.mode & FM_ATTN) {
+      plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch, tm);
+    }
+  } else {
+    // caller-supplied zoom set (sekv_decode_attn)
+    const int2 gi = __ldg(P.grp + bg);
+    span0 = gi.x; m = gi.y;
+    plan_init_fill(P, T, t, bg, span0, m);
+    int cnt = 0;
+    if (P.ids != nullptr && P.count != nullptr) cnt = max(0, min(P.count[bg], P.k_cap));
+    const int32_t* src = P.ids + (size_t)bg * max(P.k_cap, 1);
+    for (int j = T.tt; j < cnt; j += T.ts) t.sh_ids[j] = src[j];
+    cp_async_wait<0>();
+    team_bar(T);
+    plan_init_scatter(P, T, t, m);
+    team_bar(T);
+    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch);
+  }
+}
+
+// one partial record (m2, l, pad, pad, o[128]) per head
 __device__ __forceinline__ float* part_ptr(const FusedParams& P, const Item& I, int hl) {
   return P.partials + ((size_t)I.pbase + (size_t)hl * I.np + I.part) * kPartStride;
+}
+// Lane (gid, t4) holds head gid's running max m_run and its share of l_run, and the O^T accumulators
+// of[md][2 hi + c] = O[head 2 t4 + c][dim 16 md + 8 hi + gid].
+template <int G>
+__device__ __forceinline__ void store_partial(const FusedParams& P, const Item& I, int lane, float m_run, float l_run,
+                                              const float (&of)[8][4]) {
+  const int gid = lane >> 2, t4 = lane & 3;
+  l_run = quad_sum(l_run);
+  if (gid < G && t4 == 0) {
+    float* pp = part_ptr(P, I, gid);
+    pp[0] = m_run; pp[1] = l_run;
+  }
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    const int hh = 2 * t4 + c;
+    if (hh < G) {
+      float* o = part_ptr(P, I, hh) + 4 + gid;
+#pragma unroll
+      for (int md = 0; md < 8; ++md) { o[16 * md] = of[md][c]; o[16 * md + 8] = of[md][2 + c]; }
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // a5: rows [I.a, I.b) of the entry table of (b, g): pool tokens (logit = q.K/sqrt(d)) and unexpanded coarse
 // entries (logit = q.k_bar/sqrt(d) + ln|S|, value v_bar).  16-row tiles of K and V
 // stream through a kStages-deep cp.async ring in the warp's region.  Shared-memory layout of a stage:
-// K rows then V rows, 256 bytes per row, 16-byte chunk c of row r stored at chunk c ^ ((r & 1) << 2)
-// (K) or c ^ (((r >> 1) & 3) << 1) (V): both fragment access patterns below are bank-conflict free.
+// K rows then V rows, 256 bytes per row; 16-byte chunk c of row r is stored at chunk c ^ ((r & 1) << 2)
+// (K) or c ^ (r & 7) (V): both fragment access patterns below are bank-conflict free.
 //   QK^T : lane (gid = lane/4, t4 = lane%4) reads chunk (t4 + 4j) of the K row of token gid; its four
 //          words are the (b0,b1) pairs of two k-steps; Q is loaded the same way (the contraction index
 //          may be permuted consistently on both operands).
-//   P V  : computed transposed, O^T = V^T P^T (M = 16 dims, N = 8 heads, K = 16 tokens): the C fragment
-//          of S IS the B fragment of P^T.  P (fp32) is split into bf16 hi + lo parts and multiplied
-//          twice, so probabilities carry ~16 bits.
+//   P V  : computed transposed, O^T = V^T P^T (M = 16 dims, N = 8 heads, K = 16 tokens): the A fragments
+//          come from ldmatrix.trans over the V rows, the C fragment of S IS the B fragment of P^T.
+//          P (fp32) is split into bf16 hi + lo parts and multiplied twice, so probabilities carry ~16 bits.
 // ---------------------------------------------------------------------------------------------------
+// The item after a POOL item is claimed while the POOL item runs: lane 0 issues the atomic when the item starts,
+// the result is read (and the next descriptor loaded) after the first tile, so neither round trip is exposed.
+struct Ahead { int pending, nidx, n_static; bool on, done; Item nxt; };
+__device__ __forceinline__ Item load_item(const Item* p);
+__device__ __forceinline__ void ahead_resolve(const FusedParams& P, Ahead& a) {
+  if (a.on && !a.done) {
+    a.nidx = a.n_static + __shfl_sync(0xffffffffu, a.pending, 0);
+    if (a.nidx < P.main_end) a.nxt = load_item(P.items + a.nidx);
+    a.done = true;
+  }
+}
+
 template <int G>
-__device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, unsigned long long* tm) {
+__device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch,
+                                          Ahead& ah, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
   const int A = I.A, row_begin = I.a, row_end = I.b;
@@ -700,6 +746,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   const int lr = lane >> 4, lc = lane & 15;
   const uint32_t dk0 = (uint32_t)(lr * 256 + ((lc ^ (lr << 2)) << 4));
   const uint32_t dv0 = (uint32_t)(lr * 256);
+  const uint32_t lcx = (uint32_t)(lc ^ lr);
   auto fill = [&](int t) {
     uint8_t* Ks = region + (t % kStages) * kStageBytes;
     uint8_t* Vs = Ks + 16 * kD * 2;
@@ -709,7 +756,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         cp_async16(Ks + dk0 + 512 * i, Kb + src + 512 * i);
-        cp_async16(Vs + dv0 + 512 * i + ((lc ^ ((i & 3) << 1)) << 4), Vb + src + 512 * i);
+        cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src + 512 * i);
       }
     } else {
 #pragma unroll
@@ -717,7 +764,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
         const int r = 2 * i + lr;
         const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + lc * 16;
         cp_async16(Ks + dk0 + 512 * i, Kb + src);
-        cp_async16(Vs + dv0 + 512 * i + ((lc ^ ((i & 3) << 1)) << 4), Vb + src);
+        cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src);
       }
     }
   };
@@ -726,32 +773,52 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
     if (t < ntiles) fill(t);
     cp_async_commit();
   }
-  // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L.  EVERY coarse entry is
-  // included (no dependency on this step's zoom set): the ZOOM item of an expanded span subtracts that span's
-  // coarse term again (the softmax numerator and denominator are sums, "replaced by").
+  // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L (ln|S| in the base-2 domain;
+  // -inf for an expanded span, whose coarse entry is replaced by its tokens, and for rows past the item)
   float bias_reg[2] = {0.f, 0.f};
   if (I.kind == IT_COARSE) {
+    const uint2* gmask = P.zmask2 + (size_t)bg * P.mask_words;
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       const int row = row_begin + 32 * u + lane;
-      bias_reg[u] = row < row_end ? P.cv.ln_len[I.span0 + row - A] * kLog2e : -INFINITY;
+      float bias = -INFINITY;
+      if (row < row_end) {
+        const int sp = row - A;
+        const float lnl2 = P.cv.ln_len[I.span0 + sp] * kLog2e;       // (before the poll: independent of the mask)
+        bool zoomed = false;
+        if (P.k_cap > 0) {                        // poll the mask word until it carries this launch's stamp
+          uint2 w;
+          for (;;) {
+            asm volatile("ld.relaxed.gpu.global.v2.u32 {%0,%1}, [%2];" : "=r"(w.x), "=r"(w.y) : "l"(gmask + (sp >> 5)) : "memory");
+            if (w.y == epoch) break;
+            __nanosleep(64);
+          }
+          zoomed = (w.x >> (sp & 31)) & 1u;
+        }
+        if (!zoomed) bias = lnl2;
+      }
+      bias_reg[u] = bias;
     }
+    __syncwarp();
+    mark(tm, 0, lane);
   }
   uint32_t qf[4][4];
   load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
   float m_run = -INFINITY, l_run = 0.f;
-  // acc[s][w][2o + c] = O[head 2*t4 + c][dim 64s + 8gid + 2w + o]
-  float acc[2][4][4];
+  float of[8][4];
 #pragma unroll
-  for (int s = 0; s < 2; ++s)
-#pragma unroll
-    for (int w = 0; w < 4; ++w) { acc[s][w][0] = 0.f; acc[s][w][1] = 0.f; acc[s][w][2] = 0.f; acc[s][w][3] = 0.f; }
+  for (int md = 0; md < 8; ++md) { of[md][0] = 0.f; of[md][1] = 0.f; of[md][2] = 0.f; of[md][3] = 0.f; }
+  // ldmatrix.x4.trans row addresses of this lane: matrix j = lane >> 3 is tokens 8 (j >> 1) .. +7, 16-byte chunk
+  // 2 md + (j & 1) of the V rows
+  const int lj = lane >> 3, lrow = lane & 7;
+  const uint32_t v_tok_off = (uint32_t)((lrow + 8 * (lj >> 1)) * 256);
+  const uint32_t v_cx = (uint32_t)((lj & 1) ^ lrow);
 
   for (int t = 0; t < ntiles; ++t) {
     cp_async_wait<kStages - 1>();
     __syncwarp();
     const uint8_t* Ks = region + (t % kStages) * kStageBytes;
-    const uint8_t* Vs = Ks + 16 * kD * 2;
+    const uint32_t Vs = smem_u32(Ks + 16 * kD * 2) + v_tok_off;
     const int r0 = row_begin + t * 16;
     float sacc[2][4];
 #pragma unroll
@@ -784,71 +851,42 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
             bias = (ri < 32) ? b0 : b1;
           }
           if (row_begin + ri >= row_end) bias = -INFINITY;
-          z[nt][e] = fmaf(sacc[nt][e], scale2, bias);
+          z[nt][e] = (bias == -INFINITY) ? -INFINITY : fmaf(sacc[nt][e], scale2, bias);
         }
     }
     const float mx = quad_max(fmaxf(fmaxf(z[0][0], z[0][1]), fmaxf(z[1][0], z[1][1])));
     const float m_new = fmaxf(m_run, mx);
     const float m_safe = (m_new == -INFINITY) ? 0.f : m_new;
     if (__any_sync(0xffffffffu, m_new > m_run)) {
-      const float corr = exp2f(m_run - m_safe);         // this lane's head is gid
+      const float corr = ex2(m_run - m_safe);           // this lane's head is gid
       l_run *= corr;
       const float ca = __shfl_sync(0xffffffffu, corr, 8 * t4);       // head 2*t4
       const float cb = __shfl_sync(0xffffffffu, corr, 8 * t4 + 4);   // head 2*t4+1
 #pragma unroll
-      for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int w = 0; w < 4; ++w) { acc[s][w][0] *= ca; acc[s][w][1] *= cb; acc[s][w][2] *= ca; acc[s][w][3] *= cb; }
+      for (int md = 0; md < 8; ++md) { of[md][0] *= ca; of[md][1] *= cb; of[md][2] *= ca; of[md][3] *= cb; }
     }
     m_run = m_new;
-    const float p00 = exp2f(z[0][0] - m_safe), p01 = exp2f(z[0][1] - m_safe);
-    const float p10 = exp2f(z[1][0] - m_safe), p11 = exp2f(z[1][1] - m_safe);
+    const float p00 = ex2(z[0][0] - m_safe), p01 = ex2(z[0][1] - m_safe);
+    const float p10 = ex2(z[1][0] - m_safe), p11 = ex2(z[1][1] - m_safe);
     l_run += (p00 + p01) + (p10 + p11);
     uint32_t b0h, b0l, b1h, b1l;          // P^T fragments: n = head gid, k = tokens 2*t4+e (b0) and 8+2*t4+e (b1)
     split_bf16(p00, p01, b0h, b0l);
     split_bf16(p10, p11, b1h, b1l);
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      uint4 vf[4];
-#pragma unroll
-      for (int rr = 0; rr < 4; ++rr) {
-        const int r = 2 * t4 + (rr & 1) + 8 * (rr >> 1);
-        vf[rr] = *reinterpret_cast<const uint4*>(Vs + r * 256 + (((gid + 8 * s) ^ (t4 << 1)) << 4));
-      }
-      const uint32_t ra[4] = {vf[0].x, vf[0].y, vf[0].z, vf[0].w};
-      const uint32_t rb[4] = {vf[1].x, vf[1].y, vf[1].z, vf[1].w};
-      const uint32_t rc[4] = {vf[2].x, vf[2].y, vf[2].z, vf[2].w};
-      const uint32_t rd[4] = {vf[3].x, vf[3].y, vf[3].z, vf[3].w};
-#pragma unroll
-      for (int w = 0; w < 4; ++w) {
-        const uint32_t a0 = __byte_perm(ra[w], rb[w], 0x5410), a1 = __byte_perm(ra[w], rb[w], 0x7632);
-        const uint32_t a2 = __byte_perm(rc[w], rd[w], 0x5410), a3 = __byte_perm(rc[w], rd[w], 0x7632);
-        mma16816_full(acc[s][w], a0, a1, a2, a3, b0h, b1h);
-        mma16816_full(acc[s][w], a0, a1, a2, a3, b0l, b1l);
-      }
+    for (int md = 0; md < 8; ++md) {
+      uint32_t a0, a1, a2, a3;
+      ldsm_x4_trans(Vs + ((v_cx ^ (2 * md)) << 4), a0, a1, a2, a3);
+      mma16816_full(of[md], a0, a1, a2, a3, b0h, b1h);
+      mma16816_full(of[md], a0, a1, a2, a3, b0l, b1l);
     }
     __syncwarp();                                      // every lane is done with this stage
     if (t + kStages < ntiles) fill(t + kStages);
     cp_async_commit();
+    if (t == 0) ahead_resolve(P, ah);
   }
   cp_async_wait<0>();
-  l_run = quad_sum(l_run);
-  if (gid < G && t4 == 0) {
-    float* pp = part_ptr(P, I, gid);
-    pp[0] = m_run; pp[1] = l_run;
-  }
-#pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    const int hh = 2 * t4 + c;
-    if (hh < G) {
-      float* o = part_ptr(P, I, hh) + 4;
-#pragma unroll
-      for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int w = 0; w < 4; ++w)
-          *reinterpret_cast<float2*>(o + 64 * s + 8 * gid + 2 * w) = make_float2(acc[s][w][c], acc[s][w][2 + c]);
-    }
-  }
+  ahead_resolve(P, ah);
+  store_partial<G>(P, I, lane, m_run, l_run, of);
   __syncwarp();
   if (lane == 0) {
     red_add_release(grp_ctr(P, bg, C_EARLY), 1);
@@ -856,172 +894,20 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   }
 }
 
-// ---------------------------------------------------------------------------------------------------
-// a6: one expanded span, blob resident in the warp's region; the warp walks its 16-token chunks.
-//   c = sigma_K o (Vt_K q) * log2e/sqrt(d)   (rows of Vt_K play the role of tokens in QK^T)
-//   logits = U_K c  (= (U Sigma V^T q), Eq. 8 never materialised), p = 2^(z - m)
-//   y = p^T U_V,   o += (sigma_V o y) V_V^T  accumulated into the warp's running (M, L, of)
-// ---------------------------------------------------------------------------------------------------
-// NK: compile-time bound on the 16-wide k-steps over the key and value ranks (1, 2 or 4)
-template <int G, int NK>
-__device__ __forceinline__ void zoom_span_warp(const uint8_t* blob, const BlobDims& bd, int lane,
-                                               const uint32_t (&qf)[4][4], float& M, float& L, float (&of)[16][4]) {
-  const int gid = lane >> 2, t4 = lane & 3;
-  const float* sK = (const float*)(blob + bd.off_sk);
-  const float* sV = (const float*)(blob + bd.off_sv);
-  const uint8_t* VtK = blob + bd.off_vtk;
-  const uint8_t* VV = blob + bd.off_vv;
-  const int nks = (bd.rkp + 15) >> 4, nvs = (bd.rvp + 15) >> 4;     // k-steps over the key / value rank
-  const int ngrp = bd.lenp >> 4;
-  const float scale2 = rsqrtf((float)kD) * kLog2e;
-  // 1. c
-  uint32_t ckh[NK][2], ckl[NK][2];
-#pragma unroll
-  for (int ks = 0; ks < NK; ++ks) {
-    ckh[ks][0] = ckh[ks][1] = ckl[ks][0] = ckl[ks][1] = 0u;
-    if (ks < nks) {
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int nt = 2 * ks + u;
-        float cf[4] = {0.f, 0.f, 0.f, 0.f};
-        const int irow = pi_index(nt, gid);
-        const bool have = irow < bd.rkp;     // rows past the padded rank do not exist: feed zeros
-        const uint8_t* prow = VtK + (size_t)(have ? irow : 0) * (kD * 2) + t4 * 16;
-#pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
-          uint4 kv = make_uint4(0u, 0u, 0u, 0u);
-          if (have) kv = *reinterpret_cast<const uint4*>(prow + jj * 64);
-          mma16816(cf, qf[jj][0], qf[jj][1], kv.x, kv.y);
-          mma16816(cf, qf[jj][2], qf[jj][3], kv.z, kv.w);
-        }
-        // columns 2*t4+e of n-tile nt are rank index pi(nt, 2*t4+e) = 16ks + 4*t4 + 2u + e
-        const int i0 = 16 * ks + 4 * t4 + 2 * u;
-        const float s0 = (i0 < bd.rkp) ? sK[i0] * scale2 : 0.f;
-        const float s1 = (i0 + 1 < bd.rkp) ? sK[i0 + 1] * scale2 : 0.f;
-        split_bf16(cf[0] * s0, cf[1] * s1, ckh[ks][u], ckl[ks][u]);
-      }
-    }
-  }
-  // 2. the warp's token chunks
-  float m_s = -INFINITY, l_s = 0.f;
-  float yf[2 * NK][4];
-#pragma unroll
-  for (int n = 0; n < 2 * NK; ++n) { yf[n][0] = yf[n][1] = yf[n][2] = yf[n][3] = 0.f; }
-  // two 16-token chunks per iteration: their logits are independent, one running-max update serves both
-  for (int grp = 0; grp < ngrp; grp += 2) {
-    const bool two = grp + 1 < ngrp;
-    float sacc[2][2][4];
-#pragma unroll
-    for (int cc = 0; cc < 2; ++cc) {
-      const uint8_t* UKc = blob + bd.off_chunks + (size_t)(grp + cc) * bd.chunk_bytes;
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        sacc[cc][u][0] = sacc[cc][u][1] = sacc[cc][u][2] = sacc[cc][u][3] = 0.f;
-        const uint8_t* prow = UKc + (size_t)pi_index(u, gid) * (bd.rkp * 2) + t4 * 8;
-#pragma unroll
-        for (int ks = 0; ks < NK; ++ks) {
-          if (ks < nks) {
-            uint2 bv = make_uint2(0u, 0u);
-            if ((cc == 0 || two) && 16 * ks + 4 * t4 < bd.rkp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
-            mma16816(sacc[cc][u], ckh[ks][0], ckh[ks][1], bv.x, bv.y);
-            mma16816(sacc[cc][u], ckl[ks][0], ckl[ks][1], bv.x, bv.y);
-          }
-        }
-      }
-    }
-    // this lane: head gid, tokens 16 (grp + cc) + 4*t4 + 2u + e
-    float z[2][2][2];
-    float mx = -INFINITY;
-#pragma unroll
-    for (int cc = 0; cc < 2; ++cc)
-#pragma unroll
-      for (int u = 0; u < 2; ++u)
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          z[cc][u][e] = (16 * (grp + cc) + 4 * t4 + 2 * u + e < bd.len) ? sacc[cc][u][e] : -INFINITY;
-          mx = fmaxf(mx, z[cc][u][e]);
-        }
-    mx = quad_max(mx);
-    const float m_new = fmaxf(m_s, mx);
-    const float m_safe = (m_new == -INFINITY) ? 0.f : m_new;
-    if (__any_sync(0xffffffffu, m_new > m_s)) {
-      const float corr = exp2f(m_s - m_safe);
-      l_s *= corr;
-#pragma unroll
-      for (int n = 0; n < 2 * NK; ++n) { yf[n][0] *= corr; yf[n][1] *= corr; }
-    }
-    m_s = m_new;
-#pragma unroll
-    for (int cc = 0; cc < 2; ++cc) {
-      if (cc == 1 && !two) break;
-      const uint8_t* UVtc = blob + bd.off_chunks + (size_t)(grp + cc) * bd.chunk_bytes + bd.uvt_in_chunk;
-      const float p00 = exp2f(z[cc][0][0] - m_safe), p01 = exp2f(z[cc][0][1] - m_safe);
-      const float p10 = exp2f(z[cc][1][0] - m_safe), p11 = exp2f(z[cc][1][1] - m_safe);
-      l_s += (p00 + p01) + (p10 + p11);
-      uint32_t a0h, a0l, a2h, a2l;
-      split_bf16(p00, p01, a0h, a0l);     // tokens 4*t4 + {0,1}  <-> k = 2*t4 + e
-      split_bf16(p10, p11, a2h, a2l);     // tokens 4*t4 + {2,3}  <-> k = 8 + 2*t4 + e
-      // y += P U_V : B[k = token][n = i] read from the transposed factor UVt[i][token]
-#pragma unroll
-      for (int n = 0; n < 2 * NK; ++n) {
-        if (n < 2 * nvs) {
-          const int irow = pi_index(n, gid);
-          uint2 bv = make_uint2(0u, 0u);
-          if (irow < bd.rvp) bv = *reinterpret_cast<const uint2*>(UVtc + (size_t)irow * (kLenPad * 2) + t4 * 8);
-          mma16816(yf[n], a0h, a2h, bv.x, bv.y);
-          mma16816(yf[n], a0l, a2l, bv.x, bv.y);
-        }
-      }
-    }
-  }
-  // 3. fold the span into the warp's running state: of = of * 2^(M - M') + (sigma_V o y) V_V^T * 2^(m_s - M')
-  const float M_new = fmaxf(M, m_s);
-  const float M_safe = (M_new == -INFINITY) ? 0.f : M_new;
-  const float c_old = exp2f(M - M_safe), c_new = exp2f(m_s - M_safe);
-  L = fmaf(L, c_old, l_s * c_new);
-  M = M_new;
-#pragma unroll
-  for (int nd = 0; nd < 16; ++nd) { of[nd][0] *= c_old; of[nd][1] *= c_old; }
-  uint32_t yh[NK][2], yl[NK][2];          // yf[n][e] is head gid, rank index 16(n>>1) + 4*t4 + 2(n&1) + e
-#pragma unroll
-  for (int ks = 0; ks < NK; ++ks) {
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      yh[ks][u] = yl[ks][u] = 0u;
-      if (ks < nvs) {
-        const int i0 = 16 * ks + 4 * t4 + 2 * u;
-        const float s0 = (i0 < bd.rvp) ? sV[i0] * c_new : 0.f;
-        const float s1 = (i0 + 1 < bd.rvp) ? sV[i0 + 1] * c_new : 0.f;
-        split_bf16(yf[2 * ks + u][0] * s0, yf[2 * ks + u][1] * s1, yh[ks][u], yl[ks][u]);
-      }
-    }
-  }
-#pragma unroll
-  for (int nd = 0; nd < 16; ++nd) {
-    const uint8_t* prow = VV + (size_t)(8 * nd + gid) * (bd.rvp * 2) + t4 * 8;
-#pragma unroll
-    for (int ks = 0; ks < NK; ++ks) {
-      if (ks < nvs) {
-        uint2 bv = make_uint2(0u, 0u);
-        if (16 * ks + 4 * t4 < bd.rvp) bv = *reinterpret_cast<const uint2*>(prow + ks * 32);
-        mma16816(of[nd], yh[ks][0], yh[ks][1], bv.x, bv.y);
-        mma16816(of[nd], yl[ks][0], yl[ks][1], bv.x, bv.y);
-      }
-    }
-  }
-}
-
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-// lane 0 starts a 1-D bulk copy into the warp's region; every lane waits for its bytes
-__device__ __forceinline__ void region_fetch(uint8_t* region, const void* src, uint32_t bytes, uint64_t* bar,
-                                             uint32_t& phase, int lane) {
+// lane 0 starts a 1-D bulk copy into the warp's region (completion on `bar`); callers wait with mbar_wait
+__device__ __forceinline__ void region_fetch_start(uint8_t* region, const void* src, uint32_t bytes, uint64_t* bar, int lane) {
   __syncwarp();                                    // every lane is done with the region's previous contents
   if (lane == 0) {
-    fence_proxy_async_all();
+    fence_proxy_async();                           // (shared::cta) generic writes to the region before the async-proxy write
     mbar_arrive_expect_tx(bar, bytes);
     bulk_g2s(region, src, bytes, bar);
   }
+}
+__device__ __forceinline__ void region_fetch(uint8_t* region, const void* src, uint32_t bytes, uint64_t* bar,
+                                             uint32_t& phase, int lane) {
+  region_fetch_start(region, src, bytes, bar, lane);
   mbar_wait(bar, phase);
   phase ^= 1u;
 }
@@ -1042,7 +928,190 @@ __device__ __forceinline__ ZDescG poll_zdesc(const ZDescG* p, uint32_t epoch) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a4 + a6: plan items [I.a, I.b) of (b, g), one expanded span after the other through the warp's region
+// a6: one expanded span through the factored form (Eq. 8 never materialised).  Every operand is read in its
+// mma fragment order (sekv_internal.cuh): Vt_K, sigma and V_V straight from global memory (L2), the
+// per-token factors U_K, U_V from the warp's region, where they arrive by 1-D bulk copies in windows of as
+// many 16-token chunks as the region holds.
+//   c   = sigma_K o (Vt_K q) * log2e/sqrt(d)       heads x rank           (A: q,       B: Vt_K)
+//   S   = c U_K^T                                   heads x tokens         (A: c,       B: U_K)
+//   p   = 2^(S - m)
+//   y^T = U_V^T p^T                                 rank x heads           (A: U_V^T,   B: p^T = C fragment of S)
+//   O^T += V_V (sigma_V o y)^T                      dims x heads           (A: V_V,     B: y^T through movmatrix)
+// NK: compile-time bound on the 16-wide k-steps over the key and value ranks (1 or 4).
+// ---------------------------------------------------------------------------------------------------
+template <int G, int NK>
+__device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* __restrict__ blob, int len, int nks, int nvs,
+                                          uint8_t* region, uint64_t* bar, uint32_t& phase, int lane,
+                                          const uint32_t (&qf)[4][4], float& M, float& L, float (&of)[8][4],
+                                          unsigned long long* tm) {
+  // (M, L, of) are OUTPUTS: the span's own online-softmax partial (one span per ZOOM item)
+  const int gid = lane >> 2, t4 = lane & 3;
+  const size_t off_sv = (size_t)nks * 64, off_vtk = (size_t)(nks + nvs) * 64;
+  const size_t off_vv = off_vtk + (size_t)nks * 4096, off_ch = off_vv + (size_t)nvs * 4096;
+  const uint32_t chunk_bytes = (uint32_t)(nks + nvs) * 512u;
+  const int nchunks = (len + 15) >> 4;
+  const int win = max(1, min(nchunks, (int)((uint32_t)P.region_bytes / chunk_bytes)));
+  const float scale2 = rsqrtf((float)kD) * kLog2e;
+  region_fetch_start(region, blob + off_ch, (uint32_t)min(win, nchunks) * chunk_bytes, bar, lane);
+  // V_V is needed last: pull it towards L2 now
+  if (NK != 1)
+    for (int i = lane; i < nvs * 32; i += 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(blob + off_vv + (size_t)i * 128));
+  // 1. c
+  uint32_t ckh[NK][2], ckl[NK][2];
+#pragma unroll
+  for (int ks = 0; ks < NK; ++ks) {
+    ckh[ks][0] = ckh[ks][1] = ckl[ks][0] = ckl[ks][1] = 0u;
+    if (ks < nks) {
+      uint4 kv[2][4];
+#pragma unroll
+      for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) kv[u][jj] = ld_cg16(blob + off_vtk + (size_t)(((ks * 2 + u) * 4 + jj) * 512 + lane * 16));
+      const uint4 skr = ld_cg16(blob + (size_t)ks * 64 + t4 * 16);      // sigma_K[16 ks + 4 t4 .. + 3]
+      const float sk[4] = {__uint_as_float(skr.x), __uint_as_float(skr.y), __uint_as_float(skr.z), __uint_as_float(skr.w)};
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        float cf[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          mma16816(cf, qf[jj][0], qf[jj][1], kv[u][jj].x, kv[u][jj].y);
+          mma16816(cf, qf[jj][2], qf[jj][3], kv[u][jj].z, kv[u][jj].w);
+        }
+        // columns 2*t4+e of n-tile u are rank index 16 ks + 4 t4 + 2 u + e
+        split_bf16(cf[0] * (sk[2 * u] * scale2), cf[1] * (sk[2 * u + 1] * scale2), ckh[ks][u], ckl[ks][u]);
+      }
+    }
+  }
+  mark(tm, 1, lane);
+  // V_V and sigma_V are needed last: with one k-step (rank <= 16) their loads are issued now and land during the
+  // token loop (32 registers); otherwise they are loaded in the epilogue
+  uint4 vv0[8];
+  float sv0_lo = 0.f, sv0_hi = 0.f;
+  if (NK == 1) {
+#pragma unroll
+    for (int md = 0; md < 8; ++md) vv0[md] = ld_cg16(blob + off_vv + (size_t)(md * 512 + lane * 16));
+    sv0_lo = __ldcg(reinterpret_cast<const float*>(blob + off_sv) + gid);
+    sv0_hi = __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 8 + gid);
+  }
+  // 2. the token chunks, CH per iteration: their logits are independent, one running-max update serves all of
+  // them; y accumulates in two independent sets (even / odd chunks) to halve the dependent mma chain
+  constexpr int CH = NK == 1 ? 4 : 2;
+  float m_s = -INFINITY, l_s = 0.f;
+  float yf[2][NK][4];
+#pragma unroll
+  for (int a2 = 0; a2 < 2; ++a2)
+#pragma unroll
+    for (int n = 0; n < NK; ++n) { yf[a2][n][0] = yf[a2][n][1] = yf[a2][n][2] = yf[a2][n][3] = 0.f; }
+  for (int w0 = 0; w0 < nchunks; w0 += win) {
+    const int nwc = min(win, nchunks - w0);
+    mbar_wait(bar, phase);
+    phase ^= 1u;
+    for (int c = 0; c < nwc; c += CH) {
+      const int nact = min(CH, nwc - c);
+      const uint8_t* ch = region + (size_t)c * chunk_bytes + lane * 16;
+      float sacc[CH][2][4];
+#pragma unroll
+      for (int cc = 0; cc < CH; ++cc) {
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) sacc[cc][nt][0] = sacc[cc][nt][1] = sacc[cc][nt][2] = sacc[cc][nt][3] = 0.f;
+        if (cc < nact) {
+#pragma unroll
+          for (int ks = 0; ks < NK; ++ks) {
+            if (ks < nks) {
+              const uint4 bv = *reinterpret_cast<const uint4*>(ch + (size_t)cc * chunk_bytes + ks * 512);
+              mma16816(sacc[cc][0], ckh[ks][0], ckh[ks][1], bv.x, bv.y);
+              mma16816(sacc[cc][1], ckh[ks][0], ckh[ks][1], bv.z, bv.w);
+              mma16816(sacc[cc][0], ckl[ks][0], ckl[ks][1], bv.x, bv.y);
+              mma16816(sacc[cc][1], ckl[ks][0], ckl[ks][1], bv.z, bv.w);
+            }
+          }
+        }
+      }
+      // this lane: head gid, tokens 16 (w0 + c + cc) + 8 nt + 2 t4 + e
+      const int tok0 = 16 * (w0 + c);
+      if (tok0 + 16 * CH > len || nact < CH) {         // warp-uniform: only the tail needs masking
+#pragma unroll
+        for (int cc = 0; cc < CH; ++cc)
+#pragma unroll
+          for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+              if (tok0 + 16 * cc + 8 * nt + 2 * t4 + e >= len || cc >= nact) sacc[cc][nt][e] = -INFINITY;
+      }
+      float mx = -INFINITY;
+#pragma unroll
+      for (int cc = 0; cc < CH; ++cc)
+        mx = fmaxf(mx, fmaxf(fmaxf(sacc[cc][0][0], sacc[cc][0][1]), fmaxf(sacc[cc][1][0], sacc[cc][1][1])));
+      mx = quad_max(mx);
+      const float m_new = fmaxf(m_s, mx);
+      const float m_safe = (m_new == -INFINITY) ? 0.f : m_new;
+      if (__any_sync(0xffffffffu, m_new > m_s)) {
+        const float corr = ex2(m_s - m_safe);
+        l_s *= corr;
+        const float ca = __shfl_sync(0xffffffffu, corr, 8 * t4), cb = __shfl_sync(0xffffffffu, corr, 8 * t4 + 4);
+#pragma unroll
+        for (int a2 = 0; a2 < 2; ++a2)
+#pragma unroll
+          for (int n = 0; n < NK; ++n) { yf[a2][n][0] *= ca; yf[a2][n][1] *= cb; yf[a2][n][2] *= ca; yf[a2][n][3] *= cb; }
+      }
+      m_s = m_new;
+#pragma unroll
+      for (int cc = 0; cc < CH; ++cc) {
+        if (cc < nact) {
+          const float p00 = ex2(sacc[cc][0][0] - m_safe), p01 = ex2(sacc[cc][0][1] - m_safe);
+          const float p10 = ex2(sacc[cc][1][0] - m_safe), p11 = ex2(sacc[cc][1][1] - m_safe);
+          l_s += (p00 + p01) + (p10 + p11);
+          uint32_t b0h, b0l, b1h, b1l;      // P^T fragments: n = head gid, k = tokens 2 t4 + e (b0), 8 + 2 t4 + e (b1)
+          split_bf16(p00, p01, b0h, b0l);
+          split_bf16(p10, p11, b1h, b1l);
+#pragma unroll
+          for (int mv = 0; mv < NK; ++mv) {
+            if (mv < nvs) {
+              const uint4 av = *reinterpret_cast<const uint4*>(ch + (size_t)cc * chunk_bytes + (nks + mv) * 512);
+              mma16816_full(yf[cc & 1][mv], av.x, av.y, av.z, av.w, b0h, b1h);
+              mma16816_full(yf[cc & 1][mv], av.x, av.y, av.z, av.w, b0l, b1l);
+            }
+          }
+        }
+      }
+    }
+    if (w0 + win < nchunks)
+      region_fetch_start(region, blob + off_ch + (size_t)(w0 + win) * chunk_bytes,
+                         (uint32_t)min(win, nchunks - w0 - win) * chunk_bytes, bar, lane);
+  }
+  mark(tm, 2, lane);
+  // 3. O^T = V_V (sigma_V o y)^T
+  M = m_s;
+  L = l_s;
+#pragma unroll
+  for (int md = 0; md < 8; ++md) { of[md][0] = 0.f; of[md][1] = 0.f; of[md][2] = 0.f; of[md][3] = 0.f; }
+#pragma unroll
+  for (int kv = 0; kv < NK; ++kv) {
+    if (kv < nvs) {
+      // y[2 hi + c] is y^T[i = 16 kv + 8 hi + gid][head 2 t4 + c]
+      const float y0 = yf[0][kv][0] + yf[1][kv][0], y1 = yf[0][kv][1] + yf[1][kv][1];
+      const float y2 = yf[0][kv][2] + yf[1][kv][2], y3 = yf[0][kv][3] + yf[1][kv][3];
+      const float sv_lo = NK == 1 ? sv0_lo : __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 16 * kv + gid);
+      const float sv_hi = NK == 1 ? sv0_hi : __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 16 * kv + 8 + gid);
+      uint32_t h0, l0, h1, l1;
+      split_bf16(y0 * sv_lo, y1 * sv_lo, h0, l0);
+      split_bf16(y2 * sv_hi, y3 * sv_hi, h1, l1);
+      const uint32_t b0h = movmatrix_trans(h0), b1h = movmatrix_trans(h1);
+      const uint32_t b0l = movmatrix_trans(l0), b1l = movmatrix_trans(l1);
+#pragma unroll
+      for (int md = 0; md < 8; ++md) {
+        const uint4 av = NK == 1 ? vv0[md] : ld_cg16(blob + off_vv + (size_t)((kv * 8 + md) * 512 + lane * 16));
+        mma16816_full(of[md], av.x, av.y, av.z, av.w, b0h, b1h);
+        mma16816_full(of[md], av.x, av.y, av.z, av.w, b0l, b1l);
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a4 + a6: plan items [I.a, I.b) of (b, g), one expanded span after the other.  A demand miss is first
+// copied from the pinned-host store (device-mapped, over PCIe) into the cache slot the plan gave it and then
+// read from there like a hit; without a free slot it is read straight from the host store.
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
@@ -1051,69 +1120,38 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
   const int gid = lane >> 2, t4 = lane & 3;
   uint32_t qf[4][4];
   load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
-  const int j0 = I.a, j1 = I.b;                       // the plan stamps every descriptor of the schedule (id -1 = none)
+  // ONE span per ZOOM item (the plan stamps every descriptor of the schedule; id -1 = none)
   float M = -INFINITY, L = 0.f;
-  float of[16][4];
+  float of[8][4];
+  const ZDescG d = poll_zdesc(P.zdesc + (size_t)bg * P.kc + I.a, epoch);
+  mark(tm, 0, lane);
+  if (d.id >= 0) {
+    const uint8_t* blob = reinterpret_cast<const uint8_t*>(d.src);
+    if ((d.way_miss & 0xC0000000u) == 0x80000000u) {   // demand miss with a slot: pinned host -> slot, then as a hit
+      uint8_t* slot = P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFFFFFu)) * P.slot_bytes;
+      const int n16 = (int)(d.bytes >> 4);
+#pragma unroll 1
+      for (int i0 = 0; i0 < n16; i0 += 256) {
+        uint4 v[8];
 #pragma unroll
-  for (int n = 0; n < 16; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
-  const ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
-  for (int j = j0; j < j1; ++j) {
-    const ZDescG d = poll_zdesc(zd + j, epoch);
-    if (j == j0) mark(tm, 0, lane);
-    if (d.id < 0) continue;
-    // the span's coarse entry (k_bar, v_bar, ln|S|) was counted by a COARSE item: loads for taking it out again
-    const size_t crow = ((size_t)g * P.ent_head_stride + (size_t)(I.row0 + I.A + d.id) * kD) * 2;
-    const uint8_t* kbar = (const uint8_t*)P.lv.ent_k + crow;
-    const uint8_t* vbar = (const uint8_t*)P.lv.ent_v + crow;
-    uint4 kc4[4];
-    uint32_t vb[16];
+        for (int u = 0; u < 8; ++u) if (i0 + 32 * u + lane < n16) v[u] = ldg16(blob + (size_t)(i0 + 32 * u + lane) * 16);
 #pragma unroll
-    for (int jj = 0; jj < 4; ++jj) kc4[jj] = gid == 0 ? ldg16(kbar + (t4 + 4 * jj) * 16) : make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-    for (int nd = 0; nd < 16; ++nd) vb[nd] = __ldg(reinterpret_cast<const uint32_t*>(vbar + (8 * nd + 2 * t4) * 2));
-    const float lnl2 = P.cv.ln_len[I.span0 + d.id] * kLog2e;
-    region_fetch(region, (const void*)d.src, d.bytes, bar, phase, lane);
-    if (j == j0) mark(tm, 1, lane);
-    const BlobDims bd = blob_dims(2, (int)(d.len_rr >> 16), d.len_rr & 0xff, (d.len_rr >> 8) & 0xff);
-    const int kst = (max(bd.rkp, bd.rvp) + 15) >> 4;
-    if (kst <= 1) zoom_span_warp<G, 1>(region, bd, lane, qf, M, L, of);
-    else if (kst == 2) zoom_span_warp<G, 2>(region, bd, lane, qf, M, L, of);
-    else zoom_span_warp<G, 4>(region, bd, lane, qf, M, L, of);
-    {
-      // minus the coarse entry: logit z = q.k_bar/sqrt(d) + ln|S| exactly as the COARSE item computed it
-      float sacc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-      for (int jj = 0; jj < 4; ++jj) {
-        mma16816(sacc, qf[jj][0], qf[jj][1], kc4[jj].x, kc4[jj].y);
-        mma16816(sacc, qf[jj][2], qf[jj][3], kc4[jj].z, kc4[jj].w);
+        for (int u = 0; u < 8; ++u) if (i0 + 32 * u + lane < n16) *reinterpret_cast<uint4*>(slot + (size_t)(i0 + 32 * u + lane) * 16) = v[u];
       }
-      const float zc = __shfl_sync(0xffffffffu, sacc[0], lane & ~3);     // column 0 (the entry) of head gid
-      const float z = fmaf(zc, rsqrtf((float)kD) * kLog2e, lnl2);
-      const float M_new = fmaxf(M, z);
-      const float c_old = exp2f(M - M_new), w = exp2f(z - M_new);
-      M = M_new;
-      L = L * c_old - (t4 == 0 ? w : 0.f);                               // L is summed over the quad at the end
+      fence_proxy_async_all();                        // the slot is next read by the bulk-copy engine
+      __syncwarp();
+      blob = slot;
+    }
+    const int len = (int)(d.len_rr >> 16);
+    const int nks = ((int)(d.len_rr & 0xff) + 15) >> 4, nvs = ((int)((d.len_rr >> 8) & 0xff) + 15) >> 4;
+    if (nks <= 1 && nvs <= 1) zoom_span<G, 1>(P, blob, len, 1, 1, region, bar, phase, lane, qf, M, L, of, tm);
+    else zoom_span<G, 4>(P, blob, len, max(nks, 1), max(nvs, 1), region, bar, phase, lane, qf, M, L, of, tm);
+  } else {
 #pragma unroll
-      for (int nd = 0; nd < 16; ++nd) {
-        of[nd][0] = fmaf(-w, __uint_as_float(vb[nd] << 16), of[nd][0] * c_old);
-        of[nd][1] = fmaf(-w, __uint_as_float(vb[nd] & 0xffff0000u), of[nd][1] * c_old);
-      }
-    }
-    if (j == j0) mark(tm, 2, lane);
-    if ((d.way_miss & 0xC0000000u) == 0x80000000u) {   // demand miss: the blob came over PCIe; keep it in its slot
-      int4* dst = reinterpret_cast<int4*>(P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFFFFFu)) * P.slot_bytes);
-      const int4* src = reinterpret_cast<const int4*>(region);
-      for (int i = lane; i < (int)(d.bytes >> 4); i += 32) dst[i] = src[i];
-    }
+    for (int n = 0; n < 8; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
   }
   mark(tm, 3, lane);
-  L = quad_sum(L);
-  if (gid < G) {                                       // of[nd][c] is head gid, dimension 8*nd + 2*t4 + c
-    float* pp = part_ptr(P, I, gid);
-    if (t4 == 0) { pp[0] = M; pp[1] = L; }
-#pragma unroll
-    for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2*>(pp + 4 + 8 * nd + 2 * t4) = make_float2(of[nd][0], of[nd][1]);
-  }
+  store_partial<G>(P, I, lane, M, L, of);
   signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
 }
 
@@ -1144,12 +1182,12 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
     mc = warp_max(mc);
     const float Mn = fmaxf(M, mc);
     const float safe = (Mn == -INFINITY) ? 0.f : Mn;
-    const float c_old = exp2f(M - safe);
+    const float c_old = ex2(M - safe);
     // weights in parallel (lane p), kept in the record's pad word; L by a warp reduction
     float lsum = 0.f;
     for (int p = lane; p < n; p += 32) {
       const float mp = rec[p * kPartStride];
-      const float w = (mp == -INFINITY) ? 0.f : exp2f(mp - safe);
+      const float w = (mp == -INFINITY) ? 0.f : ex2(mp - safe);
       const_cast<float*>(rec)[p * kPartStride + 2] = w;
       lsum = fmaf(rec[p * kPartStride + 1], w, lsum);
     }
@@ -1165,7 +1203,7 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
     M = Mn;
     if (!second && p0 + n >= n_pool) { p0 = n_pool - cap; }     // next round starts at the first non-POOL partial
   }
-  if (!second) wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);  // (no ZOOM / COARSE partials at all)
+  if (!second) wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);  // (no ZOOM partials at all)
   const float inv = L > 0.f ? 1.f / L : 0.f;
   const size_t oi = ((size_t)b * P.Hq + (size_t)g * G + hl) * kD + 4 * lane;
   if (P.out_bf16) {
@@ -1179,11 +1217,6 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
   if (P.lse && lane == 0) P.lse[b * P.Hq + g * G + hl] = L > 0.f ? (M + log2f(L)) * kLn2 : -INFINITY;
 }
 
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
 
 __device__ __forceinline__ Item load_item(const Item* p) {
   const uint4* s = reinterpret_cast<const uint4*>(p);
@@ -1196,99 +1229,87 @@ __device__ __forceinline__ Item load_item(const Item* p) {
 }
 
 template <int G>
-__global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ FusedParams P) {
+__global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __grid_constant__ FusedParams P) {
   extern __shared__ __align__(128) uint8_t dsm[];
-  __shared__ uint64_t bars[8];
+  __shared__ uint64_t bars[kFusedWarps][2];
   __shared__ int last_flag;
-  __shared__ unsigned long long tmid_s[8 * 4];
+  __shared__ unsigned long long tmid_s[kFusedWarps * 4];
+  __shared__ int team_scratch[32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
   // Programmatic dependent launch: the next layer's grid may be scheduled as soon as this one's CTAs leave
   // their SMs (its CTAs then sit in the wait below), which hides the launch latency between the dependent
   // kernels of a step; everything this kernel touches is ordered after the previous grid by the wait.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
   uint8_t* region = dsm + (size_t)warp * P.region_bytes;
-  uint64_t* bar = &bars[warp];
-  const uint32_t epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
+  uint64_t* bar = &bars[warp][0];
   if (lane == 0) {
-    mbar_init(bar, 1);
+    mbar_init(&bars[warp][0], 1);
+    mbar_init(&bars[warp][1], 1);
     mbar_fence_init();
   }
   __syncwarp();
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const uint32_t epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
   uint32_t phase = 0u;
   unsigned long long* tm = P.trace ? &tmid_s[warp * 4] : nullptr;
 
-  // Latency items are handed out statically to the first warps of the grid (every warp of a CTA takes one), so
-  // the whole latency queue starts at t = 0; what is left of it (large batches) is claimed by the even warps,
-  // which also form the CTA's selection / plan team.  Everything else is claimed from the main queue.
-  const int nlw = (nw + 1) >> 1;
-  const int total_w = (int)gridDim.x * nw, gw = (int)blockIdx.x * nw + warp;
-  const bool team_member = (warp & 1) == 0;
-  bool in_lat = false;
-  __shared__ int team_scratch[16];
-  // selection and residency plan of this CTA's groups by the team of latency warps (once per warp)
-  auto team_work = [&]() {
+  // The chain of group bg runs on the team (warps 0 .. team_warps-1) of CTA bg % grid, starting at t = 0.  All
+  // other warps take their first work item statically (no claim latency at the start) and claim from there on.
+  const int ntw = P.team_warps;
+  const int n_chain_cta = P.has_chain ? min(P.BG, (int)gridDim.x) : 0;
+  const bool chain_cta = (int)blockIdx.x < n_chain_cta;
+  int idx;
+  if (chain_cta && warp < ntw) {
     Team T;
-    T.tt = (warp >> 1) * 32 + lane; T.ts = nlw * 32; T.lane = lane; T.tw = warp >> 1; T.ntw = nlw; T.scratch = team_scratch;
-    team_bar(T);                                               // warp 0 is done with its region (the tables live there)
+    T.tt = tid; T.ts = ntw * 32; T.lane = lane; T.tw = warp; T.ntw = ntw; T.scratch = team_scratch;
+    T.tab = dsm; T.stage = dsm + P.sm_stage + (size_t)warp * P.stage_bytes;
+    T.bars = &bars[warp][0]; T.ph[0] = 0u; T.ph[1] = 0u;
     for (int bg = (int)blockIdx.x; bg < P.BG; bg += (int)gridDim.x) {
       unsigned long long t0 = 0ull;
-      if (P.trace) { t0 = globaltimer_ns(); if (T.tt == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
-      select_team(P, T, dsm, bg, epoch, tm);
+      if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
+      chain_group<G>(P, T, bg, epoch, tm);
+#ifdef SEKV_CHAIN_TWICE
+      team_bar(T);
+      if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
+      chain_group<G>(P, T, bg, epoch, tm);
+#endif
       const int rec = P.main_end + bg;                         // trace record after the queue items
-      if (P.trace && T.tt == 0 && rec < P.trace_cap) {
+      if (P.trace && tid == 0 && rec < P.trace_cap) {
         unsigned long long* r = P.trace + 8 * (size_t)rec;
         r[0] = (unsigned long long)(uint32_t)IT_SELECT | ((unsigned long long)(uint32_t)bg << 32);
         r[1] = (unsigned long long)blockIdx.x;
         r[2] = t0; r[3] = globaltimer_ns();
         r[4] = tm[0]; r[5] = tm[1]; r[6] = tm[2]; r[7] = tm[3];
       }
-      team_bar(T);
+      team_bar(T);                                             // the tables are free for the next group
     }
-  };
+    phase = T.ph[0];                                           // the items go on with barrier 0 of this warp
+    idx = -1;
+  } else {
+    const int b = (int)blockIdx.x;
+    idx = chain_cta ? b * (nw - ntw) + (warp - ntw) : n_chain_cta * (nw - ntw) + (b - n_chain_cta) * nw + warp;
+  }
+  const int n_static = n_chain_cta * (nw - ntw) + ((int)gridDim.x - n_chain_cta) * nw;
   auto claim = [&]() -> int {
     int i = 0;
-    if (in_lat) {
-      if (lane == 0) i = P.lat_begin + total_w + atomicAdd(P.ctrs, 1);
-      i = __shfl_sync(0xffffffffu, i, 0);
-      if (i < P.lat_end) return i;
-      in_lat = false;
-      team_work();
-    }
-    if (lane == 0) i = P.lat_end + atomicAdd(P.ctrs + 1, 1);
+    if (lane == 0) i = n_static + atomicAdd(P.ctrs, 1);
     return __shfl_sync(0xffffffffu, i, 0);
   };
-  int idx;
-  if (gw < P.lat_end - P.lat_begin) {
-    idx = P.lat_begin + gw;
-    in_lat = team_member;
-  } else {
-    if (team_member) team_work();
-    idx = claim();
-  }
+  if (idx < 0) idx = claim();
   if (idx < P.main_end) {
-    // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular): the
-    // item after a POOL item is claimed, and its descriptor loaded, while the POOL item is processed.  Any
-    // other item is claimed when the warp is free to run it, so it never waits behind a slow item.
-    auto claim_after = [&](int just) -> int { return (!in_lat && just < P.pool_end) ? claim() : -1; };
+    // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular).  Any other
+    // item is claimed when the warp is free to run it, so it never waits behind a slow item.
     Item cur = load_item(P.items + idx);
-    int nidx = claim_after(idx);
     for (;;) {
-      const bool has_next = nidx >= 0 && nidx < P.main_end;
-      Item nxt = cur;
-      int nnidx = nidx;
-      if (has_next) {
-        nxt = load_item(P.items + nidx);
-        nnidx = claim_after(nidx);
-      }
+      Ahead ah;
+      ah.on = cur.kind == IT_POOL; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
+      if (ah.on && lane == 0) ah.pending = atomicAdd(P.ctrs, 1);
       unsigned long long t0 = 0ull;
       const int cur_idx = idx;
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
       switch (cur.kind) {
-        case IT_QPROJ: qproj_item<G>(P, cur, lane); break;
-        case IT_ROUTE: route_item<G>(P, cur, region, lane, tm); break;
         case IT_POOL:
-        case IT_COARSE: rows_item<G>(P, cur, region, lane, tm); break;
+        case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ah, tm); break;
         case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, epoch, tm); break;
         default: combine_item(P, cur, region, bar, phase, lane, tm); break;
       }
@@ -1301,23 +1322,21 @@ __global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ Fuse
         r[2] = t0; r[3] = globaltimer_ns();
         r[4] = tm[0]; r[5] = tm[1]; r[6] = tm[2]; r[7] = tm[3];
       }
-      if (nidx < 0) {
-        nidx = claim();
-        if (nidx >= P.main_end) break;
-        cur = load_item(P.items + nidx);
-        idx = nidx;
-        nidx = claim_after(idx);
-        continue;
+      if (ah.on) {
+        idx = ah.nidx;
+        if (idx >= P.main_end) break;
+        cur = ah.nxt;
+      } else {
+        idx = claim();
+        if (idx >= P.main_end) break;
+        cur = load_item(P.items + idx);
       }
-      if (!has_next) break;
-      cur = nxt;
-      idx = nidx;
-      nidx = nnidx;
     }
   }
   // an exiting warp has nothing left to claim, and the tail of the kernel is latency-bound: pull the tables
   // that head the next layer's dependency chain (W, routing summaries) into L2 while HBM is idle
   if (P.next_W != nullptr) {
+    const int total_w = (int)gridDim.x * nw, gw = (int)blockIdx.x * nw + warp;
     const size_t w_lines = P.next_W_bytes >> 7, r_lines = P.next_route_head_bytes >> 7;
     for (size_t i = (size_t)gw * 32 + lane; i < w_lines; i += (size_t)total_w * 32)
       asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_W + (i << 7)));
@@ -1326,7 +1345,7 @@ __global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ Fuse
       asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_route + h * P.route_head_stride * 2 + (li << 7)));
     }
   }
-  // last CTA out re-arms the queues and counters and advances the layer's step stamp
+  // last CTA out re-arms the queue and the counters and advances the layer's step stamp
   __syncthreads();
   if (tid == 0) {
     __threadfence();
@@ -1337,8 +1356,6 @@ __global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ Fuse
   if (last_flag) {
     __threadfence();
     for (int i = tid; i < 4 + 4 * P.BG; i += blockDim.x) P.ctrs[i] = 0;
-    if (P.mode & FM_ROUTE)
-      for (int i = tid; i < P.BG * G * P.dp; i += blockDim.x) reinterpret_cast<uint32_t*>(P.qp)[i] = kQpSentinel;
     if (tid == 0 && (P.mode & FM_ATTN)) {
       *P.lv.layer_step = epoch;
       atomicAdd(&P.stats[ST_LAYER_STEPS], 1ull);
@@ -1349,8 +1366,9 @@ __global__ void __maxnreg__(240) fused_layer_kernel(const __grid_constant__ Fuse
 // ---------------------------------------------------------------------------------------------------
 // a4, side stream: copy the prefetch candidates that the plan gave a slot (items n_zoom .. n_cand-1 with
 // the miss bit) from the pinned-host store into the device factor cache.  One warp per candidate; lane 0
-// drives two bulk copies through a shared-memory bounce buffer (host -> smem over PCIe, smem -> slot).
+// drives bulk copies through a shared-memory bounce buffer (host -> smem over PCIe, smem -> slot).
 // ---------------------------------------------------------------------------------------------------
+constexpr uint32_t kBounceBytes = 32768;
 __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ plan_counts,
                                                       int kc, int Hkv, int ways, int spans_cap, int64_t slot_bytes,
                                                       const uint8_t* __restrict__ host_arena) {
@@ -1367,14 +1385,22 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
     const int gs = cv.seq_span_off[b] + id;
     const int rr = lv.dir_rank[(size_t)g * spans_cap + gs];
     const uint32_t bytes = (uint32_t)blob_dims(2, cv.span_len[gs], rr & 0xff, (rr >> 8) & 0xff).bytes;
+    const uint8_t* src = host_arena + lv.dir_off[(size_t)g * spans_cap + gs];
+    uint8_t* dst = lv.slots + ((size_t)bg * ways + way) * slot_bytes;
     mbar_init(&bar, 1);
     mbar_fence_init();
-    mbar_arrive_expect_tx(&bar, bytes);
-    bulk_g2s(buf, host_arena + lv.dir_off[(size_t)g * spans_cap + gs], bytes, &bar);
-    mbar_wait(&bar, 0u);
-    fence_proxy_async();
-    bulk_s2g(lv.slots + ((size_t)bg * ways + way) * slot_bytes, buf, bytes);
-    bulk_commit();
+    uint32_t ph = 0u;
+    for (uint32_t o = 0; o < bytes; o += kBounceBytes) {
+      const uint32_t n = min(kBounceBytes, bytes - o);
+      mbar_arrive_expect_tx(&bar, n);
+      bulk_g2s(buf, src + o, n, &bar);
+      mbar_wait(&bar, ph);
+      ph ^= 1u;
+      fence_proxy_async();
+      bulk_s2g(dst + o, buf, n);
+      bulk_commit();
+      bulk_wait_read_all();
+    }
     bulk_wait_all();
   }
 }
@@ -1382,57 +1408,62 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------
-// launchers
+// host side: shared-memory plan, launchers
 // ---------------------------------------------------------------------------------------------------
 static int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
-// byte offsets of the select / plan tables inside a warp's region; returns the bytes they need
-size_t fused_plan_smem(const sekv_handle* h, FusedParams* P) {
+// byte offsets of the team's tables at the start of the CTA's dynamic shared memory; returns their size
+static size_t fused_team_tables(const sekv_handle* h, FusedParams* P) {
   const sekv_config& c = h->cfg;
   const int kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
-  size_t o = (size_t)round_up(std::max(h->max_m, 1), 4) * 4;             // keys
+  const int mm = std::max(h->max_m, 1);
+  size_t o = 0;
+  P->sm_keys = (int)o; o += (size_t)round_up(mm, 4) * 4;
   o = round_up_sz(o, 16); P->sm_hist = (int)o; o += 4 * 256 * 4;
   o = round_up_sz(o, 16); P->sm_cand = (int)o; o += (size_t)pow2_ceil(std::max(kc, 64)) * 8;
   o = round_up_sz(o, 16); P->sm_ids = (int)o; o += (size_t)kc * 4;
-  o = round_up_sz(o, 16); P->sm_wayof = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 8) * 2;
+  o = round_up_sz(o, 16); P->sm_wayof = (int)o; o += (size_t)round_up(mm, 8) * 2;
   o = round_up_sz(o, 16); P->sm_tags = (int)o; o += (size_t)c.cache_ways * 12;
   o = round_up_sz(o, 16); P->sm_mask = (int)o; o += (size_t)h->mask_words * 4;
-  o = round_up_sz(o, 16); P->sm_meta = (int)o; o += (size_t)round_up(std::max(h->max_m, 1), 4) * 4;
-  return o;
+  o = round_up_sz(o, 16); P->sm_meta = (int)o; o += (size_t)round_up(mm, 4) * 4;
+  o = round_up_sz(o, 16); P->sm_lnl = (int)o; o += (size_t)round_up(mm, 4) * 4;
+  o = round_up_sz(o, 16); P->sm_qp = (int)o; o += (size_t)h->G * c.route_dim * 4;
+  return round_up_sz(o, 128);
 }
 
-// per-warp region: the rows ring, one factor blob, or the select / plan tables
-size_t fused_region_bytes(const sekv_handle* h, FusedParams* P) {
+// Shared-memory geometry of the fused kernel for the segmented batch: per-warp regions, the team's tables and
+// routing-table staging buffers.  Returns false (with a reason) when the batch does not fit the kernel.
+bool fused_geometry(const sekv_handle* h, FusedParams* P, std::string* why) {
+  const sekv_config& c = h->cfg;
   FusedParams tmp;
   if (!P) P = &tmp;
-  size_t need = fused_plan_smem(h, P);
-  need = std::max(need, (size_t)kStages * kStageBytes);
-  if (h->cfg.k_cap > 0) need = std::max(need, (size_t)h->lay.slot_bytes);
-  need = std::max(need, (size_t)kPartStride * 4 * 8);
-  return round_up_sz(need, 128);
+  const int BG = h->n_seqs * c.n_kv_heads;
+  P->region_bytes = kRegionBytes;
+  P->team_warps = BG <= h->num_sms ? kFusedWarps : kFusedWarps / 2;
+  const size_t tables = fused_team_tables(h, P);
+  const size_t team_bytes = (size_t)P->team_warps * kRegionBytes;
+  const int per_span = h->G * c.route_dim * 2;
+  if (tables + (size_t)P->team_warps * 8 * per_span > team_bytes) {
+    if (why) *why = "select / plan tables of the longest sequence do not fit the team's shared memory";
+    return false;
+  }
+  P->sm_stage = (int)tables;
+  P->stage_bytes = (int)((team_bytes - tables) / P->team_warps / 128 * 128);
+  // spans per routing block: a multiple of 16 (mma tiles of the fast path), two buffers when they fit
+  const int fit = P->stage_bytes / per_span;
+  if (fit >= 32) { P->route_bufs = 2; P->route_spans = std::min(64, fit / 2 / 16 * 16); }
+  else if (fit >= 16) { P->route_bufs = 1; P->route_spans = 16; }
+  else if (c.route_dim != 32 && fit >= 8) { P->route_bufs = 1; P->route_spans = fit; }
+  else { if (why) *why = "routing-table staging does not fit the team's shared memory"; return false; }
+  return true;
 }
 
-// spans per ROUTE item: their G x dp rows plus q' fit the smallest region
-int fused_route_spans(const sekv_handle* h) {
-  const int per_span = h->G * h->cfg.route_dim * 2;
-  const int cap = (kStages * kStageBytes - h->G * h->cfg.route_dim * 4) / per_span;
-  return std::max(8, std::min(64, cap / 8 * 8));
-}
-
-int fused_warps(const sekv_handle* h) {
-  const size_t region = fused_region_bytes(h, nullptr);
-  const size_t budget = 227 * 1024 - 1024;
-  return (int)std::min<size_t>(8, budget / region);
-}
+int fused_warps() { return kFusedWarps; }
 
 template <int G>
 static cudaError_t launch_fused_g(const FusedParams& P, size_t smem, int grid, int threads, cudaStream_t s, bool pdl) {
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
-  }
+  cudaError_t e = cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = s;
@@ -1441,6 +1472,37 @@ static cudaError_t launch_fused_g(const FusedParams& P, size_t smem, int grid, i
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, fused_layer_kernel<G>, P);
+}
+
+template <int G>
+static cudaError_t occupancy_g(size_t smem, int threads, int* ctas_per_sm) {
+  cudaError_t e = cudaFuncSetAttribute(fused_layer_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, fused_layer_kernel<G>, threads, smem);
+}
+
+#define SEKV_DISPATCH_G(G, CALL)                 \
+  switch (G) {                                   \
+    case 1: e = CALL(1); break;                  \
+    case 2: e = CALL(2); break;                  \
+    case 3: e = CALL(3); break;                  \
+    case 4: e = CALL(4); break;                  \
+    case 5: e = CALL(5); break;                  \
+    case 6: e = CALL(6); break;                  \
+    case 7: e = CALL(7); break;                  \
+    case 8: e = CALL(8); break;                  \
+    default: e = cudaErrorInvalidValue; break;   \
+  }
+
+// The persistent kernel spins on counters published by other CTAs: every CTA of the grid must be resident.
+// Returns how many CTAs of the fused kernel one SM can hold with the current device state.
+cudaError_t fused_occupancy(const sekv_handle* h, int* ctas_per_sm) {
+  const size_t smem = (size_t)kFusedWarps * kRegionBytes;
+  cudaError_t e;
+#define OCC(GG) occupancy_g<GG>(smem, kFusedThreads, ctas_per_sm)
+  SEKV_DISPATCH_G(h->G, OCC)
+#undef OCC
+  return e;
 }
 
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
@@ -1453,9 +1515,8 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.q = (const __nv_bfloat16*)q; P.tau = tau; P.logits_out = logits; P.alpha_out = alpha;
   P.ids = ids; P.count = count; P.out = out; P.lse = lse;
   P.items = (const Item*)ws(h, h->F.off_items_sched);
+  P.grp = (const int2*)ws(h, h->F.off_bg_part);
   P.partials = (float*)ws(h, h->F.off_partials1);
-  P.keys = (uint32_t*)ws(h, h->F.off_keys);
-  P.qp = (float*)ws(h, h->F.off_qp);
   P.zdesc = (ZDescG*)ws(h, h->F.off_zdesc) + (size_t)layer * c.max_seqs * c.n_kv_heads * (std::max(c.k_cap, 1) + std::max(c.prefetch, 0));
   P.ctrs = (int32_t*)ws(h, h->F.off_ctrs) + (size_t)layer * h->F.ctrs_per_layer;
   P.plan_counts = (int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
@@ -1471,15 +1532,15 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
   P.BG = h->n_seqs * c.n_kv_heads;
   P.Hq = c.n_q_heads; P.Hkv = c.n_kv_heads; P.dp = c.route_dim; P.ways = c.cache_ways;
-  P.mask_words = h->mask_words; P.spans_cap = (int)h->lay.spans_cap; P.m_tot = h->m_tot; P.keys_stride = h->F.keys_per_bg;
+  P.mask_words = h->mask_words; P.spans_cap = (int)h->lay.spans_cap; P.m_tot = h->m_tot;
   P.out_bf16 = c.out_dtype == SEKV_BF16;
   P.slot_bytes = h->lay.slot_bytes;
   P.ent_head_stride = (size_t)h->lay.rows_cap * kD;
   P.route_head_stride = (size_t)h->lay.spans_cap * c.route_dim;
-  P.region_bytes = (int)fused_region_bytes(h, &P);
-  P.route_spans = fused_route_spans(h);
-  // queues: [QPROJ, ROUTE | SELECT | POOL, ZOOM, COARSE, COMBINE]
-  P.pool_end = h->pool_end;
+  if (!fused_geometry(h, &P, nullptr)) return cudaErrorInvalidConfiguration;
+  P.zmask2 = (uint2*)ws(h, h->F.off_zmask2) + (size_t)layer * c.max_seqs * c.n_kv_heads * h->mask_words;
+  // the chain (a1-a4) runs whenever there is routing to do or a zoom set to plan
+  P.has_chain = ((mode & FM_ROUTE) || c.k_cap > 0) ? 1 : 0;
   if ((mode & FM_ROUTE) && (mode & FM_ATTN)) {                  // whole-step launches run the layers in order
     const LayerView nv = layer_view(h, (layer + 1) % c.n_layers);
     P.next_W = (const uint8_t*)nv.W;
@@ -1487,23 +1548,13 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
     P.next_W_bytes = (size_t)c.n_q_heads * c.route_dim * kD * 2;
     P.next_route_head_bytes = (size_t)h->m_tot * c.route_dim * 2;
   }
-  if (mode == FM_ROUTE) { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_lat_items; }
-  else if (mode == FM_ATTN) { P.lat_begin = h->select_begin; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }
-  else { P.lat_begin = 0; P.lat_end = h->n_lat_items; P.main_end = h->n_items; }
-  const size_t smem = (size_t)h->fused_warps * P.region_bytes;
-  const int grid = h->fused_grid, threads = 32 * h->fused_warps;
+  P.main_end = (mode & FM_ATTN) ? h->n_items : 0;
+  const size_t smem = (size_t)kFusedWarps * kRegionBytes;
+  const int grid = h->fused_grid, threads = kFusedThreads;
   cudaError_t e;
-  switch (h->G) {
-    case 1: e = launch_fused_g<1>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 2: e = launch_fused_g<2>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 3: e = launch_fused_g<3>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 4: e = launch_fused_g<4>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 5: e = launch_fused_g<5>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 6: e = launch_fused_g<6>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 7: e = launch_fused_g<7>(P, smem, grid, threads, s, h->use_pdl); break;
-    case 8: e = launch_fused_g<8>(P, smem, grid, threads, s, h->use_pdl); break;
-    default: return cudaErrorInvalidValue;
-  }
+#define LAUNCH(GG) launch_fused_g<GG>(P, smem, grid, threads, s, h->use_pdl)
+  SEKV_DISPATCH_G(h->G, LAUNCH)
+#undef LAUNCH
   h->launches += 1;
   return e;
 }
@@ -1511,13 +1562,7 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
 cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s) {
   const sekv_config& c = h->cfg;
   if (c.prefetch <= 0 || c.k_cap <= 0) return cudaSuccess;
-  static size_t configured = 0;
-  const size_t smem = round_up_sz((size_t)h->lay.slot_bytes, 128);
-  if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(prefetch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
-  }
+  const size_t smem = std::min<size_t>(round_up_sz((size_t)h->lay.slot_bytes, 128), kBounceBytes);
   dim3 grid(c.prefetch, h->n_seqs * c.n_kv_heads);
   const int32_t* pc = (const int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
   prefetch_kernel<<<grid, 32, smem, s>>>(csr_view(h), layer_view(h, layer), pc, std::max(c.k_cap, 1) + c.prefetch,

@@ -108,15 +108,11 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   F->off_items = cv.take((size_t)NL * B * Hkv * kc * 4);
   F->off_item_span = cv.take((size_t)NL * B * Hkv * kc * 4);
   F->off_items_sched = cv.take((size_t)F->max_items * sizeof(Item));
-  F->off_bg_part = cv.take((size_t)(B * Hkv + 1) * 4);
+  F->off_bg_part = cv.take((size_t)(B * Hkv + 1) * 8);          // int2 per group: first span, span count
   F->off_bg_route = cv.take((size_t)(B * Hkv) * 4);
-  int kpb = 32;
-  while (kpb < std::min<int64_t>(mcap, SEKV_MAX_SPANS_PER_SEQ)) kpb <<= 1;
-  F->keys_per_bg = kpb;
-  F->off_keys = cv.take((size_t)B * Hkv * kpb * 8);
   F->ctrs_per_layer = (int)(4 + 4 * B * Hkv);
-  F->off_qp = cv.take((size_t)B * Hq * c.route_dim * 4);
   F->off_zdesc = cv.take((size_t)NL * B * Hkv * kc * sizeof(ZDescG));
+  F->off_zmask2 = cv.take((size_t)NL * B * Hkv * F->mask_words * 8);
   F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);
   F->off_plan_counts = cv.take((size_t)NL * B * Hkv * 2 * 4);
   F->off_layer_step = cv.take((size_t)NL * 4);
@@ -222,6 +218,84 @@ size_t sekv_blob_bytes(int32_t dtype, int32_t span_len, int32_t rank_k, int32_t 
   return blob_dims(dtype == SEKV_BF16 ? 2 : 4, span_len, rank_k, rank_v).bytes;
 }
 
+sekv_status sekv_build_sizes(const sekv_config* cfg, int32_t n_seqs, const int64_t* seq_tok_off, const float* H,
+                             sekv_sizes* out, int32_t* spans_per_seq, int32_t* pool_per_seq) {
+  if (!cfg || !out || !seq_tok_off || n_seqs < 1) return SEKV_INVALID_ARG;
+  if (cfg->l_min < 1 || cfg->r_max < 1 || cfg->r_max > SEKV_MAX_RANK || cfg->n_layers < 1 || cfg->n_kv_heads < 1 ||
+      cfg->window < 0 || !(cfg->alpha == cfg->alpha))
+    return SEKV_INVALID_ARG;
+  if (seq_tok_off[0] != 0) return SEKV_INVALID_ARG;
+  for (int b = 0; b < n_seqs; ++b)
+    if (seq_tok_off[b + 1] <= seq_tok_off[b]) return SEKV_INVALID_ARG;
+  memset(out, 0, sizeof(*out));
+  const int es = cfg->dtype == SEKV_BF16 ? 2 : 4;
+  const int64_t n_tot = seq_tok_off[n_seqs];
+  const int64_t per_store = (int64_t)cfg->n_layers * cfg->n_kv_heads;
+  out->tokens_total = n_tot;
+  if (!H) {
+    int64_t m = 0, longest = 0, bytes = 0;
+    for (int b = 0; b < n_seqs; ++b) {
+      const int64_t n = seq_tok_off[b + 1] - seq_tok_off[b];
+      const int64_t mb = n / cfg->l_min;
+      m += mb; longest = std::max(longest, n);
+      out->max_spans_per_seq = (int32_t)std::max<int64_t>(out->max_spans_per_seq, mb);
+      if (spans_per_seq) spans_per_seq[b] = (int32_t)mb;
+      if (pool_per_seq) pool_per_seq[b] = (int32_t)n;
+      // the most expensive cover of n tokens: spans of exactly l_min tokens (largest header share)
+      bytes += mb * (int64_t)blob_dims(es, cfg->l_min, std::min(cfg->r_max, cfg->l_min), std::min(cfg->r_max, cfg->l_min)).bytes
+               + (int64_t)blob_dims(es, (int)std::min<int64_t>(n, SEKV_MAX_SPAN_LEN), 1, 1).chunk_bytes;
+    }
+    if (m > INT32_MAX || n_tot > INT32_MAX) return SEKV_UNSUPPORTED;
+    out->spans_total = (int32_t)m; out->full_total = (int32_t)n_tot;
+    out->max_span_len = (int32_t)std::min<int64_t>(longest, SEKV_MAX_SPAN_LEN);
+    out->exact = 0;
+    out->host_bytes = bytes * per_store + (1 << 16);
+    return SEKV_OK;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return SEKV_CUDA; }
+  // scratch: flags (2 bytes per token), run lengths (4), token offsets, thresholds, counts, error flag
+  const size_t o_flag2 = round_up_sz((size_t)n_tot, 256), o_len = o_flag2 + round_up_sz((size_t)n_tot, 256);
+  const size_t o_off = o_len + round_up_sz((size_t)n_tot * 4, 256), o_thr = o_off + round_up_sz((size_t)(n_seqs + 1) * 8, 256);
+  const size_t o_cnt = o_thr + round_up_sz((size_t)n_seqs * 8, 256), o_err = o_cnt + round_up_sz((size_t)n_seqs * 8, 256);
+  uint8_t* tmp = nullptr;
+  if (cudaMalloc(&tmp, o_err + 256) != cudaSuccess) { cudaGetLastError(); return SEKV_OOM_DEVICE; }
+  sekv_status st = SEKV_OK;
+  std::vector<int32_t> cnt((size_t)n_seqs * 2);
+  std::vector<uint8_t> f2((size_t)n_tot);
+  std::vector<int32_t> len_at((size_t)n_tot);
+  int herr = 0;
+  cudaError_t e = cudaMemcpy(tmp + o_off, seq_tok_off, (size_t)(n_seqs + 1) * 8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess)
+    e = segment_scan(H, n_seqs, (const int64_t*)(tmp + o_off), (double)cfg->alpha, cfg->window, cfg->l_min, SEKV_MAX_SPAN_LEN,
+                     tmp, tmp + o_flag2, (int32_t*)(tmp + o_len), (double*)(tmp + o_thr), (int32_t*)(tmp + o_cnt),
+                     (int*)(tmp + o_err), 0);
+  if (e == cudaSuccess) e = cudaMemcpy(cnt.data(), tmp + o_cnt, cnt.size() * 4, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(&herr, tmp + o_err, 4, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(f2.data(), tmp + o_flag2, (size_t)n_tot, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(len_at.data(), tmp + o_len, (size_t)n_tot * 4, cudaMemcpyDeviceToHost);
+  cudaFree(tmp);
+  if (e != cudaSuccess) { cudaGetLastError(); return SEKV_CUDA; }
+  if (herr) return SEKV_UNSUPPORTED;                          // a run longer than SEKV_MAX_SPAN_LEN
+  int64_t m = 0, a = 0, bytes = 0;
+  int longest = 1;
+  for (int b = 0; b < n_seqs; ++b) {
+    a += cnt[b * 2]; m += cnt[b * 2 + 1];
+    out->max_spans_per_seq = std::max(out->max_spans_per_seq, cnt[b * 2 + 1]);
+    if (spans_per_seq) spans_per_seq[b] = cnt[b * 2 + 1];
+    if (pool_per_seq) pool_per_seq[b] = cnt[b * 2];
+  }
+  for (int64_t t = 0; t < n_tot; ++t)
+    if (f2[t] == 3) {                                          // first token of a span: its length is recorded there
+      const int len = len_at[t], r = std::min(cfg->r_max, len);
+      longest = std::max(longest, len);
+      bytes += (int64_t)blob_dims(es, len, r, r).bytes;
+    }
+  out->spans_total = (int32_t)m; out->full_total = (int32_t)a; out->max_span_len = longest; out->exact = 1;
+  out->host_bytes = bytes * per_store + (1 << 16);
+  return st;
+}
+
 sekv_status sekv_create(const sekv_config* cfg, void* device_arena, size_t device_bytes, void* host_arena,
                         size_t host_bytes, sekv_handle** out) {
   if (!out) return SEKV_INVALID_ARG;
@@ -307,12 +381,12 @@ sekv_status sekv_reset(sekv_handle* h) {
                         (std::max(c.k_cap, 1) + std::max(c.prefetch, 0)) * sizeof(ZDescG), h->main));   // stamps restart
   CK(h, cudaMemsetAsync(h->dev + F.off_stats, 0, ST_COUNT * 8, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
+  CK(h, cudaMemsetAsync(h->dev + F.off_zmask2, 0, (size_t)regions * F.mask_words * 8, h->main));      // stamps restart
   CK(h, cudaMemsetAsync(h->dev + F.off_err_flag, 0, 16, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
-  CK(h, cudaMemsetAsync(h->dev + F.off_qp, 0xFF, (size_t)c.max_seqs * c.n_q_heads * c.route_dim * 4, h->main));   // q' sentinel
   CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
-  h->n_items = h->n_lat_items = h->select_begin = 0; h->use_fused = false;
+  h->n_items = 0; h->use_fused = false; h->fused_why = "no sequences built";
   h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
   h->span_len_host.clear();
   h->m_tot = h->A_tot = h->max_m = 0;
@@ -391,35 +465,55 @@ static sekv_status make_schedule(sekv_handle* h) {
   return SEKV_OK;
 }
 
-// Work-item lists of the fused layer kernel (bf16 path), in queue order.  Latency queue: QPROJ, ROUTE (the
-// selection and plan of a group run on a team of warps once the queue is exhausted); main queue: POOL,
-// ZOOM, COARSE, COMBINE.  Both are topological orders of the dependencies (ROUTE after QPROJ, ZOOM / COARSE
-// after the group's plan, COMBINE after the attention items).
+// Work-item list of the fused layer kernel (bf16 path), in queue order: POOL, COARSE, ZOOM, COMBINE -- a
+// topological order of the dependencies (COARSE / ZOOM after the group's chain, which is not an item; COMBINE
+// after the attention items).  When the batch does not fit the kernel (or impl = 1 / fp32 storage) the generic
+// multi-kernel path runs instead and h->fused_why says why (sekv_get_path).
 static sekv_status make_fused_schedule(sekv_handle* h) {
   const FullLayout& F = h->F;
   const sekv_config& c = h->cfg;
   h->use_fused = false;
-  if (c.dtype != SEKV_BF16 || c.impl == 1) return SEKV_OK;
+  if (c.dtype != SEKV_BF16) { h->fused_why = "fp32 storage runs on the generic kernels"; return SEKV_OK; }
+  if (c.impl == 1) { h->fused_why = "impl = 1 forces the generic kernels"; return SEKV_OK; }
   const int B = h->n_seqs, Hkv = c.n_kv_heads, BG = B * Hkv, G = h->G;
-  if (h->max_m > 2048) return SEKV_OK;                      // select / plan tables live in one warp's region
-  if (c.route_dim != 8 && c.route_dim != 16 && c.route_dim != 32 && c.route_dim != 64) return SEKV_OK;
-  const int nw = fused_warps(h);
-  if (nw < 1) return SEKV_OK;                               // blobs too large for shared memory: generic path
-  h->fused_warps = nw;
-  h->fused_grid = h->num_sms;                               // one resident CTA per SM
-  int rows = c.item_rows > 0 ? c.item_rows : 128;
+  if (c.route_dim != 8 && c.route_dim != 16 && c.route_dim != 32 && c.route_dim != 64) {
+    h->fused_why = "route_dim is not 8, 16, 32 or 64"; return SEKV_OK;
+  }
+  if (!fused_geometry(h, nullptr, &h->fused_why)) return SEKV_OK;
+  // the kernel spins on counters published by other CTAs: the whole grid must be resident (one CTA per SM)
+  int per_sm = 0;
+  cudaError_t oe = fused_occupancy(h, &per_sm);
+  if (oe != cudaSuccess || per_sm < 1) {
+    cudaGetLastError();
+    h->fused_why = "the fused layer kernel cannot be resident on this device (shared memory / registers)";
+    return SEKV_OK;
+  }
+  h->fused_grid = h->num_sms;
+  FusedParams geo;
+  fused_geometry(h, &geo, nullptr);
+  const int n_chain_cta = std::min(BG, h->fused_grid);
+  const int n_first = n_chain_cta * (fused_warps() - geo.team_warps) + (h->fused_grid - n_chain_cta) * fused_warps();
+  // POOL items: by default sized so that ONE round over the warps that do not start on a chain covers every
+  // pool row (they stream while the teams run the chains)
+  int rows = c.item_rows;
+  if (rows <= 0) {
+    long pool_rows = 0;
+    for (int b = 0; b < B; ++b) pool_rows += (long)h->A_b[b] * Hkv;
+    rows = (int)((pool_rows / std::max(n_first, 1) + 1 + 15) / 16 * 16);
+    rows = std::min(256, std::max(32, rows));
+  }
   h->fused_item_rows = rows;
-  const int crows = std::min(rows, 64);
-  int zs = c.zoom_spans_per_item > 0 ? c.zoom_spans_per_item : 1;
-  const int rspans = fused_route_spans(h);
+  const int crows = 32;        // COARSE items: two tiles, both in flight while the item waits for the zoom mask
+  const int zs = 1;            // one expanded span per ZOOM item (zoom_spans_per_item is accepted and ignored)
   std::vector<Item> items;
   std::vector<int32_t> nparts(BG, 0), pbase(BG, 0);
+  std::vector<int32_t> row0(B, 0), span0(B, 0);
+  for (int b = 1; b < B; ++b) { row0[b] = row0[b - 1] + h->A_b[b - 1] + h->m_b[b - 1]; span0[b] = span0[b - 1] + h->m_b[b - 1]; }
   auto mk = [&](int kind, int b, int g, int a, int bb, int part) {
     Item it;
     memset(&it, 0, sizeof(it));
     it.kind = kind; it.bg = b * Hkv + g; it.a = a; it.b = bb; it.part = part;
-    it.A = h->A_b[b]; it.row0 = 0; it.span0 = 0;
-    for (int s = 0; s < b; ++s) { it.row0 += h->A_b[s] + h->m_b[s]; it.span0 += h->m_b[s]; }
+    it.A = h->A_b[b]; it.row0 = row0[b]; it.span0 = span0[b];
     return it;
   };
   // partial slots first (attention items need np of their group)
@@ -432,40 +526,39 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
     }
   int total_parts = 0;
   for (int bg = 0; bg < BG; ++bg) { pbase[bg] = total_parts * G; total_parts += nparts[bg]; }
-  if (total_parts > F.max_chunks) return SEKV_OK;
+  if (total_parts > F.max_chunks) { h->fused_why = "partial-record table too small for this batch"; return SEKV_OK; }
   std::vector<int32_t> next_part(BG, 0);
-  auto attn = [&](int kind, int b, int g, int a, int bb) {
+  auto attn = [&](std::vector<Item>& dst, int kind, int b, int g, int a, int bb) {
     const int bg = b * Hkv + g;
     Item it = mk(kind, b, g, a, bb, next_part[bg]++);
     it.pbase = pbase[bg]; it.np = nparts[bg];
-    items.push_back(it);
+    dst.push_back(it);
   };
+  // Queue order: [POOL: one item for every warp that does not start on a chain] [ZOOM] [COARSE] [rest of POOL]
+  // [COMBINE].  The first round of POOL items streams while the teams run the chains; the items that wait for a
+  // chain (latency-bound ZOOM first) follow, and the remaining dependency-free POOL rows fill the tail.
+  // (partial slots of a group: POOL, then COARSE, then ZOOM -- COMBINE merges the first two kinds early)
+  std::vector<Item> pool_items, coarse_items, zoom_items;
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)
-      for (int hl = 0; hl < G; ++hl) items.push_back(mk(IT_QPROJ, b, g, hl, 0, 0));
-  std::vector<int32_t> route_items(BG, 0);
-  for (int b = 0; b < B; ++b)
-    for (int g = 0; g < Hkv; ++g) {
-      const int m = h->m_b[b];
-      for (int s0 = 0; s0 < m; s0 += rspans) { items.push_back(mk(IT_ROUTE, b, g, s0, std::min(m, s0 + rspans), 0)); ++route_items[b * Hkv + g]; }
-    }
-  h->select_begin = (int)items.size();      // caller-supplied zoom sets: the latency queue is empty
-  h->n_lat_items = (int)items.size();
-  for (int b = 0; b < B; ++b)
-    for (int g = 0; g < Hkv; ++g)
-      for (int r0 = 0; r0 < h->A_b[b]; r0 += rows) attn(IT_POOL, b, g, r0, std::min(h->A_b[b], r0 + rows));
+      for (int r0 = 0; r0 < h->A_b[b]; r0 += rows) attn(pool_items, IT_POOL, b, g, r0, std::min(h->A_b[b], r0 + rows));
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g) {
       const int A = h->A_b[b], R = A + h->m_b[b];
-      for (int r0 = A; r0 < R; r0 += crows) attn(IT_COARSE, b, g, r0, std::min(R, r0 + crows));
+      for (int r0 = A; r0 < R; r0 += crows) attn(coarse_items, IT_COARSE, b, g, r0, std::min(R, r0 + crows));
     }
-  h->pool_end = (int)items.size();                    // POOL and COARSE items have no dependencies
   if (c.k_cap > 0)
     for (int b = 0; b < B; ++b)
       for (int g = 0; g < Hkv; ++g) {
         const int kmax = std::min(c.k_cap, h->m_b[b]);
-        for (int j0 = 0; j0 < kmax; j0 += zs) attn(IT_ZOOM, b, g, j0, std::min(kmax, j0 + zs));
+        for (int j0 = 0; j0 < kmax; j0 += zs) attn(zoom_items, IT_ZOOM, b, g, j0, std::min(kmax, j0 + zs));
       }
+  const size_t first = std::min<size_t>((size_t)std::max(n_first, 0), pool_items.size());
+  items.insert(items.end(), pool_items.begin(), pool_items.begin() + first);
+  h->pool_end = (int)items.size();
+  items.insert(items.end(), zoom_items.begin(), zoom_items.end());
+  items.insert(items.end(), coarse_items.begin(), coarse_items.end());
+  items.insert(items.end(), pool_items.begin() + first, pool_items.end());
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)
       for (int hl = 0; hl < G; ++hl) {
@@ -473,11 +566,16 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
         it.pbase = pbase[b * Hkv + g]; it.np = nparts[b * Hkv + g];
         items.push_back(it);
       }
-  if ((int)items.size() > F.max_items) return SEKV_OK;
+  if ((int)items.size() > F.max_items) { h->fused_why = "work-item table too small for this batch"; return SEKV_OK; }
   h->n_items = (int)items.size();
+  std::vector<int32_t> grp((size_t)BG * 2);
+  for (int b = 0; b < B; ++b)
+    for (int g = 0; g < Hkv; ++g) { grp[2 * (b * Hkv + g)] = span0[b]; grp[2 * (b * Hkv + g) + 1] = h->m_b[b]; }
+  CK(h, cudaMemcpyAsync(h->dev + F.off_bg_part, grp.data(), grp.size() * 4, cudaMemcpyHostToDevice, h->main));
   CK(h, cudaMemcpyAsync(h->dev + F.off_items_sched, items.data(), items.size() * sizeof(Item), cudaMemcpyHostToDevice, h->main));
   CK(h, cudaStreamSynchronize(h->main));
   h->use_fused = true;
+  h->fused_why.clear();
   return SEKV_OK;
 }
 
@@ -527,7 +625,7 @@ static sekv_status assign_blobs(sekv_handle* h, int layer, const std::vector<int
         return fail(h, SEKV_INVALID_ARG, "retained rank out of range (must be <= min(r_max, |S|))");
       BlobDims bd = blob_dims(h->esize, len, a, b);
       off[(size_t)g * h->lay.spans_cap + s] = (int64_t)used;
-      rank[(size_t)g * h->lay.spans_cap + s] = a | (b << 8);
+      rank[(size_t)g * h->lay.spans_cap + s] = a | (b << 8) | (len << 16);   // the fused kernel's span meta word
       used += bd.bytes;
     }
   if (used > h->host_bytes) return fail(h, SEKV_OOM_HOST, "pinned host arena too small for the factor store");
@@ -859,6 +957,7 @@ sekv_status sekv_get_stats(sekv_handle* h, sekv_stats* out) {
   out->coarse_rows_skipped = v[ST_SKIPPED];
   out->prefetched_spans = v[ST_PREFETCHED];
   out->kernel_launches = h->launches;
+  out->prefetch_h2d_bytes = v[ST_PF_BYTES];
   return SEKV_OK;
 }
 
@@ -918,6 +1017,64 @@ sekv_status sekv_set_trace(sekv_handle* h, void* buf, int64_t capacity_items, in
   for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);     // captured launches carry the old pointer
   h->graphs.clear();
   if (n_items) *n_items = h->n_items;
+  return SEKV_OK;
+}
+
+sekv_status sekv_get_path(const sekv_handle* h, int32_t* fused, const char** reason) {
+  if (!h) return SEKV_INVALID_ARG;
+  if (fused) *fused = h->use_fused ? 1 : 0;
+  if (reason) *reason = h->fused_why.c_str();
+  return SEKV_OK;
+}
+
+sekv_status sekv_export_span_factors(sekv_handle* h, int32_t layer, int32_t seq, int32_t kv_head, int32_t span,
+                                     int32_t* len_out, int32_t* rank_k, int32_t* rank_v, float* UK, float* sK,
+                                     float* VtK, float* UV, float* sV, float* VtV, int32_t* pad_zero) {
+  if (!h) return SEKV_INVALID_ARG;
+  sekv_status s = check_ready(h, layer);
+  if (s != SEKV_OK) return s;
+  const sekv_config& c = h->cfg;
+  if (seq < 0 || seq >= h->n_seqs || kv_head < 0 || kv_head >= c.n_kv_heads) return fail(h, SEKV_INVALID_ARG, "sequence or kv head out of range");
+  if (span < 0 || span >= h->m_b[seq]) return fail(h, SEKV_INVALID_ARG, "span out of range");
+  int gs = span;
+  for (int b = 0; b < seq; ++b) gs += h->m_b[b];
+  LayerView lv = layer_view(h, layer);
+  int64_t off = 0;
+  int32_t rr = 0;
+  CK(h, cudaStreamSynchronize(h->main));
+  CK(h, cudaMemcpy(&off, lv.dir_off + (size_t)kv_head * h->lay.spans_cap + gs, 8, cudaMemcpyDeviceToHost));
+  CK(h, cudaMemcpy(&rr, lv.dir_rank + (size_t)kv_head * h->lay.spans_cap + gs, 4, cudaMemcpyDeviceToHost));
+  const int len = h->span_len_host[gs], rk = rr & 0xff, rv = (rr >> 8) & 0xff, es = h->esize;
+  if (len_out) *len_out = len;
+  if (rank_k) *rank_k = rk;
+  if (rank_v) *rank_v = rv;
+  const BlobDims bd = blob_dims(es, len, rk, rv);
+  const uint8_t* blob = h->host + off;
+  auto ld = [&](size_t o) -> float {
+    if (es == 4) { float v; memcpy(&v, blob + o, 4); return v; }
+    uint16_t u; memcpy(&u, blob + o, 2);
+    uint32_t w = (uint32_t)u << 16; float v; memcpy(&v, &w, 4); return v;
+  };
+  const float* bsk = (const float*)(blob + bd.off_sk);
+  const float* bsv = (const float*)(blob + bd.off_sv);
+  if (sK) for (int i = 0; i < rk; ++i) sK[i] = bsk[i];
+  if (sV) for (int i = 0; i < rv; ++i) sV[i] = bsv[i];
+  if (VtK) for (int i = 0; i < rk; ++i) for (int d = 0; d < kD; ++d) VtK[(size_t)i * kD + d] = ld(blob_vtk_off(bd, es, i, d));
+  if (VtV) for (int i = 0; i < rv; ++i) for (int d = 0; d < kD; ++d) VtV[(size_t)i * kD + d] = ld(blob_vv_off(bd, es, d, i));
+  if (UK) for (int t = 0; t < len; ++t) for (int i = 0; i < rk; ++i) UK[(size_t)t * rk + i] = ld(blob_uk_off(bd, es, t, i));
+  if (UV) for (int t = 0; t < len; ++t) for (int i = 0; i < rv; ++i) UV[(size_t)t * rv + i] = ld(blob_uv_off(bd, es, t, i));
+  if (pad_zero) {
+    bool ok = true;
+    for (int i = rk; i < bd.rkp; ++i) ok = ok && bsk[i] == 0.f;
+    for (int i = rv; i < bd.rvp; ++i) ok = ok && bsv[i] == 0.f;
+    for (int i = 0; i < bd.rkp && ok; ++i) for (int d = 0; d < kD; ++d) if (i >= rk && ld(blob_vtk_off(bd, es, i, d)) != 0.f) ok = false;
+    for (int i = 0; i < bd.rvp && ok; ++i) for (int d = 0; d < kD; ++d) if (i >= rv && ld(blob_vv_off(bd, es, d, i)) != 0.f) ok = false;
+    for (int t = 0; t < bd.lenp && ok; ++t) {
+      for (int i = 0; i < bd.rkp; ++i) if ((t >= len || i >= rk) && ld(blob_uk_off(bd, es, t, i)) != 0.f) ok = false;
+      for (int i = 0; i < bd.rvp; ++i) if ((t >= len || i >= rv) && ld(blob_uv_off(bd, es, t, i)) != 0.f) ok = false;
+    }
+    *pad_zero = ok ? 1 : 0;
+  }
   return SEKV_OK;
 }
 

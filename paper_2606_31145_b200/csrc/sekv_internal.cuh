@@ -13,7 +13,7 @@
 namespace sekv {
 
 constexpr int kD = SEKV_HEAD_DIM;   // d_h
-constexpr int kRankPad = 8;         // ranks padded to a multiple of this in a blob
+constexpr int kRankPad = 16;        // ranks padded to a multiple of this in a blob (one mma k-step)
 constexpr int kLenPad = 16;         // |S| padded to a multiple of this in a blob
 constexpr int kTile = 16;           // stage-1 schedules entry rows in tiles of 16
 constexpr int kPartStride = kD + 4; // floats per partial: m2, l, pad, pad, o[128]
@@ -23,13 +23,20 @@ __host__ __device__ inline int round_up(int x, int m) { return (x + m - 1) / m *
 __host__ __device__ inline size_t round_up_sz(size_t x, size_t m) { return (x + m - 1) / m * m; }
 
 // ---- factor blob layout ------------------------------------------------
-// header : [sigma_K f32 rkp][sigma_V f32 rvp][VtK st rkp x 128][VV st 128 x rvp]
-// chunks : lenp/16 chunks of 16 tokens, each [UK st 16 x rkp][UVt st rvp x 16]
-// Each operand is stored with its contraction index contiguous; a chunk is one contiguous piece, so a
-// whole blob (or any run of chunks) moves with a single 1-D bulk copy (cp.async.bulk).
+// Every operand is stored in the FRAGMENT ORDER of the warp-level mma.sync.m16n8k16 that consumes it in
+// the fused layer kernel: a block of 32 lanes x 16 bytes (8 elements) per fragment load, lane = 4 gid + t4,
+// so that each load is one 16-byte access per lane at consecutive addresses (coalesced from global memory,
+// bank-conflict free from shared memory).  nks / nvs = ceil(rank_k / 16), ceil(rank_v / 16).
+//   header : [sigma_K f32 16 nks][sigma_V f32 16 nvs]
+//            [VtK : nks x (2 u x 4 jj) blocks]   B operand of c = Vt_K q   (rows = rank index, cols = d)
+//            [VV  : nvs x 8 md blocks]           A operand of O^T = V_V (sigma_V o y)^T
+//   chunks : ceil(|S| / 16) chunks of 16 tokens, each [U_K : nks blocks][U_V : nvs blocks]
+//            U_K = B operand of S = c U_K^T, U_V = A operand of y^T = U_V^T P^T
+// The header and any run of chunks are contiguous pieces (1-D bulk copies).  Element positions are given by
+// the blob_*_off functions below; the pack kernel, the generic kernels and the export go through them.
 struct BlobDims {
-  int len, lenp, rk, rv, rkp, rvp;
-  size_t off_sk, off_sv, off_vtk, off_vv, off_chunks, chunk_bytes, uvt_in_chunk, bytes;
+  int len, lenp, rk, rv, rkp, rvp, nks, nvs;
+  size_t off_sk, off_sv, off_vtk, off_vv, off_chunks, chunk_bytes, bytes;
 };
 __host__ __device__ inline BlobDims blob_dims(int esize, int len, int rk, int rv) {
   BlobDims b;
@@ -37,24 +44,48 @@ __host__ __device__ inline BlobDims blob_dims(int esize, int len, int rk, int rv
   b.lenp = round_up(len, kLenPad);
   b.rkp = round_up(rk > 0 ? rk : 1, kRankPad);
   b.rvp = round_up(rv > 0 ? rv : 1, kRankPad);
+  b.nks = b.rkp / 16; b.nvs = b.rvp / 16;
   size_t o = 0;
   b.off_sk = o;  o += (size_t)b.rkp * 4;
   b.off_sv = o;  o += (size_t)b.rvp * 4;
   b.off_vtk = o; o += (size_t)b.rkp * kD * esize;
   b.off_vv = o;  o += (size_t)kD * b.rvp * esize;
   b.off_chunks = o;
-  b.uvt_in_chunk = (size_t)kLenPad * b.rkp * esize;
   b.chunk_bytes = (size_t)kLenPad * (b.rkp + b.rvp) * esize;
   o += (size_t)(b.lenp / kLenPad) * b.chunk_bytes;
   b.bytes = round_up_sz(o, 128);
   return b;
 }
-// byte offset of U_K[t][i] and of U_V[t][i] (stored transposed inside the chunk) within a blob
-__host__ __device__ inline size_t blob_uk_off(const BlobDims& b, int esize, int t, int i) {
-  return b.off_chunks + (size_t)(t / kLenPad) * b.chunk_bytes + ((size_t)(t % kLenPad) * b.rkp + i) * esize;
+// byte offset of Vt_K[i][d] (i = rank index): block (ks, u, jj), lane (gid, t4), element e8 with
+// i = 16 ks + 4 (gid >> 1) + 2 u + (gid & 1),  d = 32 jj + 8 t4 + e8
+__host__ __device__ inline size_t blob_vtk_off(const BlobDims& b, int esize, int i, int d) {
+  const int ks = i >> 4, il = i & 15;
+  const int u = (il >> 1) & 1, gid = 2 * (il >> 2) + (il & 1);
+  const int jj = d >> 5, t4 = (d & 31) >> 3, e8 = d & 7;
+  return b.off_vtk + ((size_t)((((ks * 2 + u) * 4 + jj) * 32 + gid * 4 + t4) * 8 + e8)) * esize;
 }
+// byte offset of V_V[d][i] = Vt_V[i][d]: block (kv, md), lane (gid, t4), register a_{2 half + hi}, element e with
+// d = 16 md + 8 hi + gid,  i = 16 kv + 8 half + 2 t4 + e
+__host__ __device__ inline size_t blob_vv_off(const BlobDims& b, int esize, int d, int i) {
+  const int kv = i >> 4, il = i & 15;
+  const int half = il >> 3, t4 = (il & 7) >> 1, e = il & 1;
+  const int md = d >> 4, hi = (d & 15) >> 3, gid = d & 7;
+  return b.off_vv + ((size_t)(((kv * 8 + md) * 32 + gid * 4 + t4) * 8 + (half * 2 + hi) * 2 + e)) * esize;
+}
+// byte offset of U_K[t][i]: chunk t / 16, block ks, lane (gid, t4), n-tile nt, element e4 with
+// t = 16 c + 8 nt + gid,  i = 16 ks + 4 t4 + e4
+__host__ __device__ inline size_t blob_uk_off(const BlobDims& b, int esize, int t, int i) {
+  const int tl = t & 15, nt = tl >> 3, gid = tl & 7;
+  const int ks = i >> 4, t4 = (i & 15) >> 2, e4 = i & 3;
+  return b.off_chunks + (size_t)(t >> 4) * b.chunk_bytes + ((size_t)((ks * 32 + gid * 4 + t4) * 8 + nt * 4 + e4)) * esize;
+}
+// byte offset of U_V[t][i]: chunk t / 16, block nks + mv, lane (gid, t4), register a_{2 half + hi}, element e with
+// t = 16 c + 8 half + 2 t4 + e,  i = 16 mv + 8 hi + gid
 __host__ __device__ inline size_t blob_uv_off(const BlobDims& b, int esize, int t, int i) {
-  return b.off_chunks + (size_t)(t / kLenPad) * b.chunk_bytes + b.uvt_in_chunk + ((size_t)i * kLenPad + (t % kLenPad)) * esize;
+  const int tl = t & 15, half = tl >> 3, t4 = (tl & 7) >> 1, e = tl & 1;
+  const int mv = i >> 4, hi = (i & 15) >> 3, gid = i & 7;
+  return b.off_chunks + (size_t)(t >> 4) * b.chunk_bytes +
+         ((size_t)(((b.nks + mv) * 32 + gid * 4 + t4) * 8 + (half * 2 + hi) * 2 + e)) * esize;
 }
 
 // ---- device views ------------------------------------------------------------------------------
@@ -100,19 +131,20 @@ struct Chunk {  // one stage-1 work item
   int32_t part;       // partial slot within the head
 };
 
-enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_PREFETCHED, ST_COUNT = 8 };
+enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FACTOR_ALGO, ST_SKIPPED, ST_PREFETCHED, ST_PF_BYTES, ST_COUNT = 10 };
 
 // ---- fused layer kernel (fused_kernels.cu) -------------------------------------------------------
-// Work items of the per-layer persistent kernel.  Every item is processed by ONE warp.  Two queues:
-//   latency queue : ROUTE (Eq. 4-5), SELECT (Eq. 9 top-k + factor-cache plan)
-//   main queue    : POOL, ZOOM, COARSE (L119-121, Eq. 8), COMBINE (L61)
+// Work items of the per-layer persistent kernel.  Every item is processed by ONE warp, claimed in queue order:
+// POOL, COARSE (L119-121), ZOOM (Eq. 8), COMBINE (L61).  The chain a1-a4 of a group (q' = W q, routing scores,
+// top-k, factor-cache plan) is not an item: a team of warps runs it at the start of the kernel (IT_SELECT is its
+// trace record).
 enum ItemKind { IT_QPROJ = 0, IT_ROUTE = 1, IT_SELECT = 2, IT_POOL = 3, IT_ZOOM = 4, IT_COARSE = 5, IT_COMBINE = 6 };
 enum FusedMode { FM_ROUTE = 1, FM_ATTN = 2 };   // FM_ATTN without FM_ROUTE: caller-supplied zoom set
 struct __align__(16) Item {   // 48 bytes: three 16-byte loads
   int32_t kind;        // ItemKind
   int32_t bg;          // b * H_kv + g
-  int32_t a, b;        // QPROJ/COMBINE: a = head within the group; ROUTE: span range; SELECT: a = route items of
-                       // the group, b = m; POOL / COARSE: entry-row range; ZOOM: plan-item range
+  int32_t a, b;        // COMBINE: a = head within the group, b = POOL + COARSE partials; POOL / COARSE: entry-row
+                       // range; ZOOM: plan-item range
   int32_t part;        // partial slot within the group (attention items)
   int32_t A;           // pool rows of the sequence
   int32_t row0;        // first entry row of the sequence
@@ -144,12 +176,10 @@ struct FusedParams {
   void* out;                   // [B][H][128]
   float* lse;                  // [B][H] or null
   const Item* items;
+  const int2* grp;             // [BG] first span and span count of the group's sequence
   float* partials;             // records [pbase + hl * np + part][kPartStride]
-  uint32_t* keys;              // [BG][keys_stride] ordered routing keys (0 = not eligible)
-  float* qp;                   // [BG][G][dp] projected queries
   ZDescG* zdesc;               // [BG][kc] of this layer
-  int32_t* ctrs;               // [0] latency queue, [1] main queue, [2] exited CTAs, [3] pad, then per group:
-                               // qp_done, route_done, attn_done, plan_flag
+  int32_t* ctrs;               // [0] work queue, [2] exited CTAs, then per group: early_done, -, attn_done, plan_flag
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
   unsigned long long* stats;
   const uint8_t* host_arena;   // device alias of the pinned host factor store
@@ -159,13 +189,15 @@ struct FusedParams {
   size_t next_W_bytes, next_route_head_bytes;
   size_t ent_head_stride, route_head_stride;
   int64_t slot_bytes, trace_cap;
-  int32_t lat_begin, lat_end, main_end;         // item index ranges of the two queues
-  int32_t pool_end;                              // first main-queue item that is not a POOL item
+  uint2* zmask2;               // [BG][mask_words] (zoom bits, step stamp) pairs of this layer
+  int32_t main_end;                              // number of work items of this launch
   int32_t mode, k, k_cap, prefetch, kc, BG;
-  int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, keys_stride, out_bf16;
+  int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, out_bf16;
   int32_t region_bytes;                          // per-warp shared-memory region
-  int32_t route_spans;                           // spans per ROUTE item
-  int32_t sm_cand, sm_ids, sm_wayof, sm_tags, sm_mask, sm_hist, sm_meta;   // byte offsets in the region (select / plan)
+  int32_t team_warps, has_chain;                 // warps 0 .. team_warps-1 of CTA bg % grid run the chain of group bg
+  int32_t route_spans, route_bufs;               // spans per routing block, staging buffers per team warp (1 or 2)
+  int32_t sm_stage, stage_bytes;                 // staging buffers: dsm + sm_stage + warp * stage_bytes
+  int32_t sm_keys, sm_cand, sm_ids, sm_wayof, sm_tags, sm_mask, sm_hist, sm_meta, sm_lnl, sm_qp;   // team tables (byte offsets)
 };
 
 // ---- storage-type helpers ------------------------------------------------------------------------
@@ -222,8 +254,8 @@ struct FullLayout {
   int64_t off_partials1, off_partials2, off_ws_ids, off_ws_count, off_stats, off_chunks, off_bg_chunk,
       off_zoom_mask, off_items, off_item_span, off_layer_step, off_seg_flag, off_seg_flag2, off_seg_len,
       off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag, off_items_sched, off_bg_part,
-      off_bg_route, off_keys, off_ctrs, off_plan_counts, off_qp, off_zdesc;
-  int mask_words, max_chunks, max_items, ctrs_per_layer, keys_per_bg;
+      off_bg_route, off_ctrs, off_plan_counts, off_zdesc, off_zmask2;
+  int mask_words, max_chunks, max_items, ctrs_per_layer;
   size_t total;
 };
 
@@ -252,7 +284,8 @@ struct sekv_handle {
   int n_chunks, parts1_max, P2, parts_per_head, sort_n;
   // fused layer kernel (bf16 path)
   bool use_fused, use_pdl;
-  int n_items, n_lat_items, select_begin, pool_end, fused_grid, fused_warps, fused_item_rows;
+  std::string fused_why;             // why the batch runs on the generic path (empty when use_fused)
+  int n_items, pool_end, fused_grid, fused_item_rows;
   int num_sms;
   std::vector<GraphEntry> graphs;
   uint64_t launches;
@@ -283,6 +316,9 @@ LayerView layer_view(const sekv_handle* h, int layer);
 // launchers (each returns the cudaError_t of the launch)
 cudaError_t launch_segment(sekv_handle* h, const float* H, int n_seqs, const int64_t* tok_off_host,
                            int* m_out, int* a_out, std::string* why);
+cudaError_t segment_scan(const float* H, int n_seqs, const int64_t* tok_off_dev, double alpha, int window, int l_min,
+                         int max_span_len, uint8_t* flag, uint8_t* flag2, int32_t* len_at, double* thr,
+                         int32_t* counts, int* err, cudaStream_t s);
 cudaError_t launch_build_prefactored(sekv_handle* h, int layer, const float* H, const sekv_factors* f,
                                      const void* W);
 cudaError_t launch_build_dense(sekv_handle* h, int layer, const float* H, const void* K, const void* V,
@@ -297,9 +333,9 @@ cudaError_t launch_combine(sekv_handle* h, int layer, void* out, float* lse, cud
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
                          float* alpha, int32_t* ids, int32_t* count, void* out, float* lse, cudaStream_t s);
 cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s);
-size_t fused_region_bytes(const sekv_handle* h, FusedParams* P);
-int fused_warps(const sekv_handle* h);
-int fused_route_spans(const sekv_handle* h);
+bool fused_geometry(const sekv_handle* h, FusedParams* P, std::string* why);
+cudaError_t fused_occupancy(const sekv_handle* h, int* ctas_per_sm);
+int fused_warps();
 
 inline uint8_t* ws(const sekv_handle* h, int64_t off) { return h->dev + off; }
 

@@ -14,36 +14,28 @@ from . import binding as B
 def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Optional[int] = None,
                out_dtype: str = "f32", use_graph: int = 0, impl: int = 0, stage1_ctas: int = 0,
                r_max: Optional[int] = None, slack: float = 1.0, prefetch: int = 0, item_rows: int = 0,
-               zoom_spans_per_item: int = 0) -> B.sekv_config:
-    m_tot = sum(l.m for l in layouts)
-    a_tot = sum(l.A for l in layouts)
-    n_tot = sum(l.n for l in layouts)
-    max_m = max(l.m for l in layouts)
-    max_len = max(int(l.planted_span_len.max()) if l.m else 1 for l in layouts)
+               zoom_spans_per_item: int = 0, H_dev: Optional[torch.Tensor] = None, device="cuda:0"):
+    """(sekv_config, pinned host bytes) for a batch.  Capacities come from sekv_build_sizes, i.e. from what a
+    real caller has: the token counts and the surprisal tensor -- never from the generator's planted layout."""
+    if H_dev is None:
+        H_dev = surprisal_device(layouts, device)
+    base = dict(n_layers=spec.n_layers, n_q_heads=spec.n_q_heads, n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim,
+                route_dim=spec.route_dim, dtype=B.SEKV_BF16 if spec.dtype == "bf16" else B.SEKV_F32,
+                out_dtype=B.SEKV_BF16 if out_dtype == "bf16" else B.SEKV_F32, alpha=spec.alpha, l_min=spec.l_min,
+                r_max=r_max or spec.rank, window=spec.window, max_seqs=len(layouts))
+    sz, _, _ = B.sekv_build_sizes(B.make_config(**base), seq_tok_off(layouts), H_dev)
     if k_cap is None:
-        k_cap = max_m if spec.top_k < 0 else spec.top_k
+        k_cap = sz.max_spans_per_seq if spec.top_k < 0 else spec.top_k
     if spec.top_k < 0:
         prefetch = 0
     if cache_ways is None:
         cache_ways = max(2 * (k_cap + prefetch), 1) if spec.top_k >= 0 else max(k_cap, 1)
-    return B.make_config(
-        n_layers=spec.n_layers, n_q_heads=spec.n_q_heads, n_kv_heads=spec.n_kv_heads, head_dim=spec.head_dim,
-        route_dim=spec.route_dim, dtype=B.SEKV_BF16 if spec.dtype == "bf16" else B.SEKV_F32,
-        out_dtype=B.SEKV_BF16 if out_dtype == "bf16" else B.SEKV_F32, alpha=spec.alpha, l_min=spec.l_min,
-        r_max=r_max or spec.rank, window=spec.window, max_seqs=len(layouts), max_tokens_total=n_tot,
-        max_spans_total=int(m_tot * slack) + 1, max_full_total=int(a_tot * slack) + 1,
-        max_span_len=min(1024, -(-max(max_len, 16) // 16) * 16), k_cap=k_cap, cache_ways=max(cache_ways, 1),
-        prefetch=prefetch, stage1_ctas=stage1_ctas, item_rows=item_rows, zoom_spans_per_item=zoom_spans_per_item,
-        use_graph=use_graph, impl=impl)
-
-
-def host_bytes_for(spec, layouts, cfg: B.sekv_config) -> int:
-    total = 0
-    for l in layouts:
-        for ln in l.planted_span_len:
-            r = min(spec.rank, int(ln))
-            total += B.sekv_blob_bytes(cfg.dtype, int(ln), r, r)
-    return total * spec.n_kv_heads * spec.n_layers + (1 << 16)
+    cfg = B.make_config(
+        **base, max_tokens_total=sz.tokens_total, max_spans_total=int(sz.spans_total * slack) + 1,
+        max_full_total=int(sz.full_total * slack) + 1, max_span_len=min(1024, -(-max(sz.max_span_len, 16) // 16) * 16),
+        k_cap=k_cap, cache_ways=max(cache_ways, 1), prefetch=prefetch, stage1_ctas=stage1_ctas, item_rows=item_rows,
+        zoom_spans_per_item=zoom_spans_per_item, use_graph=use_graph, impl=impl)
+    return cfg, int(sz.host_bytes)
 
 
 def seq_tok_off(layouts) -> list:
@@ -68,9 +60,9 @@ def create_engine(spec, layouts, device="cuda:0", mode: str = "prefactored", gen
                   layer_inputs: Optional[Sequence] = None, **cfg_kw) -> B.Sekv:
     """Create a handle sized for `spec` and build every layer from the seeded generator."""
     from workloads import make_layer_inputs
-    cfg = config_for(spec, layouts, **cfg_kw)
-    eng = B.Sekv(cfg, host_bytes_for(spec, layouts, cfg), device=device)
-    H_dev = surprisal_device(layouts, eng.device)
+    H_dev = surprisal_device(layouts, device)
+    cfg, host_bytes = config_for(spec, layouts, H_dev=H_dev, device=device, **cfg_kw)
+    eng = B.Sekv(cfg, host_bytes, device=device)
     gdev = gen_device or "cpu"
     for layer in range(spec.n_layers):
         li = layer_inputs[layer] if layer_inputs is not None else make_layer_inputs(

@@ -1,6 +1,7 @@
-"""sekv_export_tables: decode the library's stored tables (device arena + pinned host arena) into
-plain numpy arrays in the paper's orientation, for tests and the timed CPU baseline.  Pure format
-decoding driven by sekv_get_layout -- no arithmetic of the method."""
+"""sekv_export_tables: the library's stored tables as plain numpy arrays in the paper's orientation, for
+tests.  The row-major device tables are sliced out of the arena with the offsets of sekv_get_layout; the factor
+blobs (stored in mma fragment order) are decoded by the library (sekv_export_span_factors).  No arithmetic of
+the method."""
 from __future__ import annotations
 
 from typing import Dict, List
@@ -17,24 +18,6 @@ def _view(arena: torch.Tensor, off: int, nbytes: int, dtype: torch.dtype) -> tor
 
 def _f64(t: torch.Tensor) -> np.ndarray:
     return t.detach().to(torch.float32).cpu().numpy().astype(np.float64)
-
-
-def blob_sections(esize: int, ln: int, rk: int, rv: int) -> dict:
-    """Byte offsets of a factor blob; mirrors the layout stated in sekv_internal.cuh:
-    header [sK f32 rkp][sV f32 rvp][VtK rkp x 128][VV 128 x rvp], then lenp/16 chunks of 16 tokens,
-    each [UK 16 x rkp][UVt rvp x 16]."""
-    lenp = -(-ln // 16) * 16
-    rkp = -(-max(rk, 1) // 8) * 8
-    rvp = -(-max(rv, 1) // 8) * 8
-    o = 0
-    sec = {"lenp": lenp, "rkp": rkp, "rvp": rvp}
-    sec["sk"] = o; o += rkp * 4
-    sec["sv"] = o; o += rvp * 4
-    sec["vtk"] = o; o += rkp * 128 * esize
-    sec["vv"] = o; o += 128 * rvp * esize
-    sec["chunks"] = o; o += lenp * (rkp + rvp) * esize
-    sec["bytes"] = -(-o // 128) * 128
-    return sec
 
 
 def export_tables(eng: B.Sekv, layer: int, b: int, with_factors: bool = True) -> Dict:
@@ -72,29 +55,15 @@ def export_tables(eng: B.Sekv, layer: int, b: int, with_factors: bool = True) ->
     out["route_K"] = _f64(route[:, s0:s1])
     out["W"] = _f64(_view(dev, lay.w + layer * lay.w_layer_stride, Hq * dp * 128 * es, st).view(Hq, dp, 128))
     if with_factors:
-        n_dir = lay.dir_layer_stride_elems
-        dir_off = _view(dev, lay.dir_off + layer * n_dir * 8, n_dir * 8, torch.int64).view(Hkv, lay.spans_cap).cpu().numpy()
-        dir_rank = _view(dev, lay.dir_rank + layer * n_dir * 4, n_dir * 4, torch.int32).view(Hkv, lay.spans_cap).cpu().numpy()
-        host = eng.host_arena
+        # the blob layout (mma fragment order) is decoded by the library itself: sekv_export_span_factors
         factors: List[List[dict]] = []
         for g in range(Hkv):
             row = []
-            for s in range(s0, s1):
-                ln = int(span_len[s]); rk = int(dir_rank[g, s]) & 0xff; rv = (int(dir_rank[g, s]) >> 8) & 0xff
-                sec = blob_sections(es, ln, rk, rv)
-                blob = host[int(dir_off[g, s]):int(dir_off[g, s]) + sec["bytes"]]
-                sK = blob[sec["sk"]:sec["sk"] + sec["rkp"] * 4].view(torch.float32)
-                sV = blob[sec["sv"]:sec["sv"] + sec["rvp"] * 4].view(torch.float32)
-                VtK = blob[sec["vtk"]:sec["vtk"] + sec["rkp"] * 128 * es].view(st).view(sec["rkp"], 128)
-                VV = blob[sec["vv"]:sec["vv"] + 128 * sec["rvp"] * es].view(st).view(128, sec["rvp"])
-                ch = blob[sec["chunks"]:sec["chunks"] + sec["lenp"] * (sec["rkp"] + sec["rvp"]) * es].view(st)
-                ch = ch.view(sec["lenp"] // 16, 16 * (sec["rkp"] + sec["rvp"]))
-                UK = ch[:, :16 * sec["rkp"]].reshape(sec["lenp"], sec["rkp"])                       # [lenp][rkp]
-                UVt = ch[:, 16 * sec["rkp"]:].reshape(sec["lenp"] // 16, sec["rvp"], 16).permute(1, 0, 2).reshape(sec["rvp"], sec["lenp"])
-                row.append(dict(UK=_f64(UK[:ln, :rk]), sK=_f64(sK[:rk]), VtK=_f64(VtK[:rk]),
-                                UV=_f64(UVt[:rv, :ln]).T.copy(), sV=_f64(sV[:rv]), VtV=_f64(VV[:, :rv]).T.copy(),
-                                pad_ok=bool((UK[ln:].float() == 0).all() and (UVt[:, ln:].float() == 0).all()
-                                            and (sK[rk:] == 0).all() and (sV[rv:] == 0).all())))
+            for s in range(m):
+                f = eng.sekv_export_span_factors(layer, b, g, s)
+                row.append(dict(UK=f["UK"].astype(np.float64), sK=f["sK"].astype(np.float64),
+                                VtK=f["VtK"].astype(np.float64), UV=f["UV"].astype(np.float64),
+                                sV=f["sV"].astype(np.float64), VtV=f["VtV"].astype(np.float64), pad_ok=f["pad_ok"]))
             factors.append(row)
         out["factors"] = factors
     return out

@@ -28,7 +28,9 @@ def test_header_declares_the_named_entry_points():
     syms = _declared_symbols()
     for name in ("sekv_build_spans", "sekv_route", "sekv_decode_attn", "sekv_create", "sekv_destroy"):
         assert name in syms
-    assert len(syms) >= 18
+    for name in ("sekv_build_sizes", "sekv_get_path", "sekv_export_span_factors"):
+        assert name in syms
+    assert len(syms) >= 21
 
 
 def test_library_exports_every_declared_symbol(binding):
@@ -41,16 +43,21 @@ def test_pure_entry_points(binding):
     B = binding
     assert "sm_100a" in B.sekv_version()
     assert B.lib.sekv_status_string(0) == b"SEKV_OK" and B.lib.sekv_status_string(6) == b"SEKV_STATE"
-    # blob bytes: PAPER.md L108 count r(|S| + d_h + 1) for K and V, fp32 sigma, ranks padded to 8, |S| to 16
+    # blob bytes: PAPER.md L108 count r(|S| + d_h + 1) for K and V, fp32 sigma, ranks and |S| padded to 16
     for dtype, es in ((B.SEKV_BF16, 2), (B.SEKV_F32, 4)):
         for ln, rk, rv in ((256, 16, 16), (100, 16, 16), (16, 4, 8), (77, 33, 64)):
-            lp, kp, vp = -(-ln // 16) * 16, -(-rk // 8) * 8, -(-rv // 8) * 8
+            lp, kp, vp = -(-ln // 16) * 16, -(-rk // 16) * 16, -(-rv // 16) * 16
             raw = 4 * (kp + vp) + es * (128 * (kp + vp) + lp * (kp + vp))
             assert B.sekv_blob_bytes(dtype, ln, rk, rv) == -(-raw // 128) * 128
             algo = (rk + rv) * (ln + 128) * es + 4 * (rk + rv)
             assert B.sekv_blob_bytes(dtype, ln, rk, rv) >= algo
     cfg = B.make_config(n_layers=2, max_seqs=2, max_tokens_total=10000, max_spans_total=100, max_full_total=300,
                         k_cap=8, cache_ways=16, r_max=16)
+    # sizes from token counts alone (no GPU): m_b <= n_b / l_min, A_b <= n_b
+    sz, spans, pool = B.sekv_build_sizes(cfg, [0, 4096, 10000])
+    assert not sz.exact and sz.tokens_total == 10000 and sz.full_total == 10000
+    assert spans == [4096 // 16, 5904 // 16] and pool == [4096, 5904] and sz.spans_total == sum(spans)
+    assert sz.max_span_len == 1024 and sz.host_bytes >= 2 * 8 * sum(spans) * B.sekv_blob_bytes(B.SEKV_BF16, 16, 16, 16)
     dev, slot = B.sekv_device_arena_bytes(cfg)
     assert slot == B.sekv_blob_bytes(B.SEKV_BF16, 256, 16, 16)
     assert dev > 2 * 2 * 8 * 16 * slot          # at least the factor cache
