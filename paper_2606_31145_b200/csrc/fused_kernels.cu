@@ -97,6 +97,14 @@ __device__ __forceinline__ uint4 ld_cg16(const void* p) {       // L2-coherent 1
   return v;
 }
 
+// header loads of a ZOOM item: the header is in a cache slot (global) or, for a demand miss, staged in shared memory
+__device__ __forceinline__ uint4 hdr_ld16(const uint8_t* p, bool in_smem) {
+  return in_smem ? *reinterpret_cast<const uint4*>(p) : ld_cg16(p);
+}
+__device__ __forceinline__ float hdr_ldf(const uint8_t* p, bool in_smem) {
+  return in_smem ? *reinterpret_cast<const float*>(p) : __ldcg(reinterpret_cast<const float*>(p));
+}
+
 // per-group counters inside P.ctrs
 __device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
 enum { C_EARLY = 0, C_ATTN = 2 };   // C_EARLY: POOL + COARSE items done, C_ATTN: every attention item done
@@ -200,10 +208,12 @@ __device__ __forceinline__ void qproj_mma(const FusedParams& P, int hl, int j0, 
 }
 
 // meta = |S| << 16 | rank_k | rank_v << 8 of the span
+// it = way | miss << 31 | no-slot << 30; j = index of the span in the sorted zoom list (the ZOOM item's partial slot)
 __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, int bg, int g, int span0, int id, uint32_t it,
-                                            uint32_t meta, uint32_t epoch) {
+                                            uint32_t meta, uint32_t epoch, int j = 0) {
   ZDescG d;
-  d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = it; d.id = id; d.epoch0 = epoch; d.epoch1 = epoch;
+  d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = (it & 0xC0003FFFu) | ((uint32_t)j << 14); d.id = id;
+  d.epoch0 = epoch; d.epoch1 = epoch;
   if (id >= 0) {
     const int gs = span0 + id;
     const int rr = (int)(meta & 0xffffu);
@@ -213,7 +223,7 @@ __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, in
     // hits: the cache slot; misses: the device alias of the pinned-host store (the ZOOM item copies the blob into
     // its slot first when it has one)
     const uint8_t* src = (it & 0x80000000u) ? P.host_arena + P.lv.dir_off[(size_t)g * P.spans_cap + gs]
-                                            : P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFFFFFu)) * P.slot_bytes;
+                                            : P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFu)) * P.slot_bytes;
     d.src = (unsigned long long)src;
   }
   uint4* o = reinterpret_cast<uint4*>(zd);
@@ -258,6 +268,7 @@ __device__ __forceinline__ void plan_init_fill(const FusedParams& P, const Team&
   }
   cp_async_commit();
   for (int w = T.tt; w < P.mask_words; w += T.ts) t.sh_mask[w] = 0u;
+  if (T.tt == 0) { T.scratch[24] = 0; T.scratch[25] = 0; T.scratch[26] = 0; }   // descriptor positions (plan_team)
 }
 __device__ __forceinline__ void plan_init_scatter(const FusedParams& P, const Team& T, const PlanTables& t, int m) {
   for (int w = T.tt; w < P.ways; w += T.ts) { const int tg = t.sh_tag[w]; if (tg >= 0 && tg < m) t.way_of[tg] = (int16_t)w; }
@@ -441,10 +452,20 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   int32_t* item_span = P.lv.item_span + (size_t)bg * P.kc;
   ZDescG* zd = P.zdesc + (size_t)bg * P.kc;
   const uint32_t cur = epoch;
+  // Descriptor positions of the zoom set: ZOOM item i of the group polls zd[i], and the items are claimed in
+  // that order.  Demand misses (slowest: their blob crosses PCIe) take the first positions; hits and "none"
+  // entries fill the positions from the back.  Every list index j < K gets exactly one descriptor, which
+  // carries j: the partial of span j always lands in slot j, so the merge order -- and the output bits -- do not
+  // depend on which position (or warp) a span went to.  Prefetch candidate c is zd[kcap1 + c].
+  const int K = min(P.k_cap, m);
+  int* pos_hit = T.scratch + 24; int* pos_miss = T.scratch + 25;
   int n_hit = 0, n_miss = 0, n_pf = 0, n_pf_slot = 0;
   unsigned long long bytes_algo = 0, bytes_demand = 0, bytes_pf = 0;
   // pass 1: validate / de-duplicate, zoom mask, residency lookup
-  for (int j = T.tt; j < n_cand; j += T.ts) {
+  for (int j = T.tt; j < max(n_cand, K); j += T.ts) {
+    if (j >= n_zoom && j < K)                                  // list index past the zoom set: "none", done at once
+      write_zdesc(P, zd + (K - 1 - atomicAdd(pos_hit, 1)), bg, g, span0, -1, 0u, 0u, epoch, j);
+    if (j >= n_cand) continue;
     int id = t.sh_ids[j];
     if (id < 0 || id >= m) id = -1;
     const bool zoom = j < n_zoom;
@@ -470,11 +491,11 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
     t.sh_ids[j] = id;
     item_span[j] = id;
     items[j] = (way >= 0) ? (uint32_t)way : 0xFFFFFFFFu;
-    // hits (and dropped duplicates) publish their descriptor at once: the ZOOM items poll it and start
-    // while the misses are still being given slots
-    if (zoom && (way >= 0 || id < 0)) write_zdesc(P, zd + j, bg, g, span0, id, (uint32_t)max(way, 0), meta, epoch);
+    // hits publish their descriptor at once: the ZOOM items poll it and start while the misses are still
+    // being given slots; a resident prefetch candidate needs no copy
+    if (zoom && (way >= 0 || id < 0))
+      write_zdesc(P, zd + (K - 1 - atomicAdd(pos_hit, 1)), bg, g, span0, id, (uint32_t)max(way, 0), meta, epoch, j);
   }
-  for (int j = n_zoom + T.tt; j < min(P.k_cap, m); j += T.ts) write_zdesc(P, zd + j, bg, g, span0, -1, 0u, 0u, epoch);
   int n_need;
   team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1 to the team)
   n_need = min(n_need, ways);
@@ -526,7 +547,7 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
       items[j] = it;
     }
     miss_base += tot;
-    if (miss && j < n_zoom) write_zdesc(P, zd + j, bg, g, span0, id, it, t.meta[id], epoch);
+    if (miss && j < n_zoom) write_zdesc(P, zd + atomicAdd(pos_miss, 1), bg, g, span0, id, it, t.meta[id], epoch, j);
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
@@ -940,22 +961,31 @@ __device__ __forceinline__ ZDescG poll_zdesc(const ZDescG* p, uint32_t epoch) {
 // NK: compile-time bound on the 16-wide k-steps over the key and value ranks (1 or 4).
 // ---------------------------------------------------------------------------------------------------
 template <int G, int NK>
-__device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* __restrict__ blob, int len, int nks, int nvs,
-                                          uint8_t* region, uint64_t* bar, uint32_t& phase, int lane,
+__device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* __restrict__ blob, const uint8_t* hdr,
+                                          bool hdr_smem, int len, int nks, int nvs, uint8_t* region, uint32_t cap_bytes,
+                                          uint64_t* bar, uint32_t& phase, int lane,
                                           const uint32_t (&qf)[4][4], float& M, float& L, float (&of)[8][4],
-                                          unsigned long long* tm) {
+                                          uint8_t* wb, bool wb_regs, unsigned long long* tm) {
+  // blob: where the chunk windows come from (cache slot, or the pinned-host copy of a demand miss); hdr: the header
+  // (= blob, or a copy staged in shared memory); region / cap_bytes: where the windows go.
+  // wb: null, or the cache slot a demand miss is kept in: the chunk windows are written to it by bulk copies out
+  // of the region (and, with wb_regs, the header pieces this warp holds in registers by plain stores).
   // (M, L, of) are OUTPUTS: the span's own online-softmax partial (one span per ZOOM item)
   const int gid = lane >> 2, t4 = lane & 3;
   const size_t off_sv = (size_t)nks * 64, off_vtk = (size_t)(nks + nvs) * 64;
   const size_t off_vv = off_vtk + (size_t)nks * 4096, off_ch = off_vv + (size_t)nvs * 4096;
   const uint32_t chunk_bytes = (uint32_t)(nks + nvs) * 512u;
   const int nchunks = (len + 15) >> 4;
-  const int win = max(1, min(nchunks, (int)((uint32_t)P.region_bytes / chunk_bytes)));
+  // (windows hold a multiple of CH chunks, so the iterations group the same chunks whatever the window size:
+  // a span gives the same bits from a cache slot and from the host store)
+  constexpr int CH = NK == 1 ? 4 : 2;
+  const int fit = (int)(cap_bytes / chunk_bytes);
+  const int win = max(1, min(nchunks, fit >= CH ? fit / CH * CH : fit));
   const float scale2 = rsqrtf((float)kD) * kLog2e;
   region_fetch_start(region, blob + off_ch, (uint32_t)min(win, nchunks) * chunk_bytes, bar, lane);
   // V_V is needed last: pull it towards L2 now
-  if (NK != 1)
-    for (int i = lane; i < nvs * 32; i += 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(blob + off_vv + (size_t)i * 128));
+  if (NK != 1 && !hdr_smem)
+    for (int i = lane; i < nvs * 32; i += 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(hdr + off_vv + (size_t)i * 128));
   // 1. c
   uint32_t ckh[NK][2], ckl[NK][2];
 #pragma unroll
@@ -966,8 +996,16 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
 #pragma unroll
       for (int u = 0; u < 2; ++u)
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) kv[u][jj] = ld_cg16(blob + off_vtk + (size_t)(((ks * 2 + u) * 4 + jj) * 512 + lane * 16));
-      const uint4 skr = ld_cg16(blob + (size_t)ks * 64 + t4 * 16);      // sigma_K[16 ks + 4 t4 .. + 3]
+        for (int jj = 0; jj < 4; ++jj) kv[u][jj] = hdr_ld16(hdr + off_vtk + (size_t)(((ks * 2 + u) * 4 + jj) * 512 + lane * 16), hdr_smem);
+      const uint4 skr = hdr_ld16(hdr + (size_t)ks * 64 + t4 * 16, hdr_smem);      // sigma_K[16 ks + 4 t4 .. + 3]
+      if (wb && wb_regs) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj)
+            *reinterpret_cast<uint4*>(wb + off_vtk + (size_t)(((ks * 2 + u) * 4 + jj) * 512 + lane * 16)) = kv[u][jj];
+        if (gid == 0) *reinterpret_cast<uint4*>(wb + (size_t)ks * 64 + t4 * 16) = skr;
+      }
       const float sk[4] = {__uint_as_float(skr.x), __uint_as_float(skr.y), __uint_as_float(skr.z), __uint_as_float(skr.w)};
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
@@ -989,13 +1027,20 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
   float sv0_lo = 0.f, sv0_hi = 0.f;
   if (NK == 1) {
 #pragma unroll
-    for (int md = 0; md < 8; ++md) vv0[md] = ld_cg16(blob + off_vv + (size_t)(md * 512 + lane * 16));
-    sv0_lo = __ldcg(reinterpret_cast<const float*>(blob + off_sv) + gid);
-    sv0_hi = __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 8 + gid);
+    for (int md = 0; md < 8; ++md) vv0[md] = hdr_ld16(hdr + off_vv + (size_t)(md * 512 + lane * 16), hdr_smem);
+    sv0_lo = hdr_ldf(hdr + off_sv + 4 * gid, hdr_smem);
+    sv0_hi = hdr_ldf(hdr + off_sv + 4 * (8 + gid), hdr_smem);
+    if (wb && wb_regs) {
+#pragma unroll
+      for (int md = 0; md < 8; ++md) *reinterpret_cast<uint4*>(wb + off_vv + (size_t)(md * 512 + lane * 16)) = vv0[md];
+      if (t4 == 0) {
+        reinterpret_cast<float*>(wb + off_sv)[gid] = sv0_lo;
+        reinterpret_cast<float*>(wb + off_sv)[8 + gid] = sv0_hi;
+      }
+    }
   }
   // 2. the token chunks, CH per iteration: their logits are independent, one running-max update serves all of
   // them; y accumulates in two independent sets (even / odd chunks) to halve the dependent mma chain
-  constexpr int CH = NK == 1 ? 4 : 2;
   float m_s = -INFINITY, l_s = 0.f;
   float yf[2][NK][4];
 #pragma unroll
@@ -1006,6 +1051,10 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
     const int nwc = min(win, nchunks - w0);
     mbar_wait(bar, phase);
     phase ^= 1u;
+    if (wb && lane == 0) {                             // keep the window: region -> slot (async, read-only on the region)
+      bulk_s2g(wb + off_ch + (size_t)w0 * chunk_bytes, region, (uint32_t)nwc * chunk_bytes);
+      bulk_commit();
+    }
     for (int c = 0; c < nwc; c += CH) {
       const int nact = min(CH, nwc - c);
       const uint8_t* ch = region + (size_t)c * chunk_bytes + lane * 16;
@@ -1075,10 +1124,13 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
         }
       }
     }
-    if (w0 + win < nchunks)
+    if (w0 + win < nchunks) {
+      if (wb && lane == 0) bulk_wait_read_all();        // the write-back has read the region
       region_fetch_start(region, blob + off_ch + (size_t)(w0 + win) * chunk_bytes,
                          (uint32_t)min(win, nchunks - w0 - win) * chunk_bytes, bar, lane);
+    }
   }
+  if (wb && lane == 0) bulk_wait_all();
   mark(tm, 2, lane);
   // 3. O^T = V_V (sigma_V o y)^T
   M = m_s;
@@ -1091,8 +1143,12 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
       // y[2 hi + c] is y^T[i = 16 kv + 8 hi + gid][head 2 t4 + c]
       const float y0 = yf[0][kv][0] + yf[1][kv][0], y1 = yf[0][kv][1] + yf[1][kv][1];
       const float y2 = yf[0][kv][2] + yf[1][kv][2], y3 = yf[0][kv][3] + yf[1][kv][3];
-      const float sv_lo = NK == 1 ? sv0_lo : __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 16 * kv + gid);
-      const float sv_hi = NK == 1 ? sv0_hi : __ldcg(reinterpret_cast<const float*>(blob + off_sv) + 16 * kv + 8 + gid);
+      const float sv_lo = NK == 1 ? sv0_lo : hdr_ldf(hdr + off_sv + 4 * (16 * kv + gid), hdr_smem);
+      const float sv_hi = NK == 1 ? sv0_hi : hdr_ldf(hdr + off_sv + 4 * (16 * kv + 8 + gid), hdr_smem);
+      if (NK != 1 && wb && wb_regs && t4 == 0) {
+        reinterpret_cast<float*>(wb + off_sv)[16 * kv + gid] = sv_lo;
+        reinterpret_cast<float*>(wb + off_sv)[16 * kv + 8 + gid] = sv_hi;
+      }
       uint32_t h0, l0, h1, l1;
       split_bf16(y0 * sv_lo, y1 * sv_lo, h0, l0);
       split_bf16(y2 * sv_hi, y3 * sv_hi, h1, l1);
@@ -1100,7 +1156,8 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
       const uint32_t b0l = movmatrix_trans(l0), b1l = movmatrix_trans(l1);
 #pragma unroll
       for (int md = 0; md < 8; ++md) {
-        const uint4 av = NK == 1 ? vv0[md] : ld_cg16(blob + off_vv + (size_t)((kv * 8 + md) * 512 + lane * 16));
+        const uint4 av = NK == 1 ? vv0[md] : hdr_ld16(hdr + off_vv + (size_t)((kv * 8 + md) * 512 + lane * 16), hdr_smem);
+        if (NK != 1 && wb && wb_regs) *reinterpret_cast<uint4*>(wb + off_vv + (size_t)((kv * 8 + md) * 512 + lane * 16)) = av;
         mma16816_full(of[md], av.x, av.y, av.z, av.w, b0h, b1h);
         mma16816_full(of[md], av.x, av.y, av.z, av.w, b0l, b1l);
       }
@@ -1127,32 +1184,74 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
   mark(tm, 0, lane);
   if (d.id >= 0) {
     const uint8_t* blob = reinterpret_cast<const uint8_t*>(d.src);
-    if ((d.way_miss & 0xC0000000u) == 0x80000000u) {   // demand miss with a slot: pinned host -> slot, then as a hit
-      uint8_t* slot = P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFFFFFu)) * P.slot_bytes;
-      const int n16 = (int)(d.bytes >> 4);
-#pragma unroll 1
-      for (int i0 = 0; i0 < n16; i0 += 256) {
-        uint4 v[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) if (i0 + 32 * u + lane < n16) v[u] = ldg16(blob + (size_t)(i0 + 32 * u + lane) * 16);
-#pragma unroll
-        for (int u = 0; u < 8; ++u) if (i0 + 32 * u + lane < n16) *reinterpret_cast<uint4*>(slot + (size_t)(i0 + 32 * u + lane) * 16) = v[u];
-      }
-      fence_proxy_async_all();                        // the slot is next read by the bulk-copy engine
-      __syncwarp();
-      blob = slot;
-    }
     const int len = (int)(d.len_rr >> 16);
-    const int nks = ((int)(d.len_rr & 0xff) + 15) >> 4, nvs = ((int)((d.len_rr >> 8) & 0xff) + 15) >> 4;
-    if (nks <= 1 && nvs <= 1) zoom_span<G, 1>(P, blob, len, 1, 1, region, bar, phase, lane, qf, M, L, of, tm);
-    else zoom_span<G, 4>(P, blob, len, max(nks, 1), max(nvs, 1), region, bar, phase, lane, qf, M, L, of, tm);
+    const int nks = max(1, ((int)(d.len_rr & 0xff) + 15) >> 4), nvs = max(1, ((int)((d.len_rr >> 8) & 0xff) + 15) >> 4);
+    // Demand miss: the blob is read from the pinned-host store over PCIe by the bulk-copy engine only (plain loads
+    // of host memory turn into many 32-byte PCIe reads): first the header into the front of the region (and on into
+    // the slot, when the plan gave it one), then the chunk windows behind it, each kept in the slot on the way.
+    const bool miss = (d.way_miss & 0x80000000u) != 0u;
+    uint8_t* wb = nullptr;
+    if ((d.way_miss & 0xC0000000u) == 0x80000000u) wb = P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFu)) * P.slot_bytes;
+    const uint32_t hdr_bytes = (uint32_t)(nks + nvs) * (64u + 4096u), chunk_bytes = (uint32_t)(nks + nvs) * 512u;
+    const uint8_t* hdr = blob;
+    uint8_t* cbase = region;
+    uint32_t cap = (uint32_t)P.region_bytes;
+    bool hdr_smem = false, wb_regs = wb != nullptr;
+    if (miss && hdr_bytes + chunk_bytes <= (uint32_t)P.region_bytes) {
+      region_fetch(region, blob, hdr_bytes, bar, phase, lane);
+      if (wb && lane == 0) { bulk_s2g(wb, region, hdr_bytes); bulk_commit(); }
+      hdr = region; hdr_smem = true; wb_regs = false;
+      cbase = region + hdr_bytes; cap = (uint32_t)P.region_bytes - hdr_bytes;
+    }
+    if (nks <= 1 && nvs <= 1) zoom_span<G, 1>(P, blob, hdr, hdr_smem, len, 1, 1, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, tm);
+    else zoom_span<G, 4>(P, blob, hdr, hdr_smem, len, nks, nvs, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, tm);
   } else {
 #pragma unroll
     for (int n = 0; n < 8; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
   }
   mark(tm, 3, lane);
-  store_partial<G>(P, I, lane, M, L, of);
+  Item Ij = I;                                                   // the partial of list index j goes to slot j
+  Ij.part = I.part - I.a + (int)((d.way_miss >> 14) & 0xFFFFu);
+  store_partial<G>(P, Ij, lane, M, L, of);
   signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// a4, speculative prefetch: candidate I.a of group (b, g) of the PREVIOUS layer of this step -- one of the
+// next-best spans by routing score that was not resident and that the previous layer's plan gave a slot -- is
+// copied pinned host -> slot by the bulk-copy engine, bounced through the warp's region.  The previous layer's
+// kernel is complete (plain loads of its plan), its cache is next read one step later, and the copy has this
+// whole kernel to cross PCIe: it is on nobody's critical path.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void prefetch_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
+                                              uint32_t& phase, int lane) {
+  const int bg = I.bg, g = bg % P.Hkv;
+  const int j = P.pf_plan_counts[2 * bg] + I.a;
+  if (j >= P.pf_plan_counts[2 * bg + 1]) return;
+  const int id = P.pf_lv.item_span[(size_t)bg * P.kc + j];
+  const uint32_t it = P.pf_lv.items[(size_t)bg * P.kc + j];
+  if (id < 0 || (it & 0xC0000000u) != 0x80000000u) return;
+  const int gs = I.span0 + id;
+  const uint32_t rr = (uint32_t)P.pf_lv.dir_rank[(size_t)g * P.spans_cap + gs];   // |S| << 16 | r_V << 8 | r_K
+  const uint32_t bytes = (uint32_t)blob_dims(2, (int)(rr >> 16), rr & 0xff, (rr >> 8) & 0xff).bytes;
+  const uint8_t* src = P.host_arena + P.pf_lv.dir_off[(size_t)g * P.spans_cap + gs];
+  uint8_t* dst = P.pf_lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFu)) * P.slot_bytes;
+  __syncwarp();
+  if (lane == 0) {
+    const uint32_t piece = (uint32_t)P.region_bytes;
+    for (uint32_t o = 0; o < bytes; o += piece) {
+      const uint32_t n = min(piece, bytes - o);
+      mbar_arrive_expect_tx(bar, n);
+      bulk_g2s(region, src + o, n, bar);
+      mbar_wait(bar, phase);
+      phase ^= 1u;
+      bulk_s2g(dst + o, region, n);
+      bulk_commit();
+      bulk_wait_read_all();                          // the region may be overwritten by the next piece
+    }
+    bulk_wait_all();
+  }
+  phase = __shfl_sync(0xffffffffu, phase, 0);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1311,6 +1410,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
         case IT_POOL:
         case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ah, tm); break;
         case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, epoch, tm); break;
+        case IT_PREFETCH: if (P.pf_plan_counts != nullptr) prefetch_item(P, cur, region, bar, phase, lane); break;
         default: combine_item(P, cur, region, bar, phase, lane, tm); break;
       }
       if (P.trace && lane == 0 && cur_idx < P.trace_cap) {
@@ -1364,9 +1464,9 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
 }
 
 // ---------------------------------------------------------------------------------------------------
-// a4, side stream: copy the prefetch candidates that the plan gave a slot (items n_zoom .. n_cand-1 with
-// the miss bit) from the pinned-host store into the device factor cache.  One warp per candidate; lane 0
-// drives bulk copies through a shared-memory bounce buffer (host -> smem over PCIe, smem -> slot).
+// The same copies as prefetch_item by a kernel of their own, for the cases in which no following layer kernel
+// can carry them: a one-layer model, or a caller that reads the last layer's cache before the next step.
+// One warp per candidate; lane 0 drives bulk copies through a shared-memory bounce buffer.
 // ---------------------------------------------------------------------------------------------------
 constexpr uint32_t kBounceBytes = 32768;
 __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, const int32_t* __restrict__ plan_counts,
@@ -1374,19 +1474,18 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
                                                       const uint8_t* __restrict__ host_arena) {
   extern __shared__ __align__(128) uint8_t buf[];
   __shared__ uint64_t bar;
-  const int bg = blockIdx.y, b = bg / Hkv, g = bg % Hkv;
+  const int bg = blockIdx.y, g = bg % Hkv;
   const int j = plan_counts[2 * bg] + blockIdx.x;
   if (j >= plan_counts[2 * bg + 1]) return;
   const int id = lv.item_span[(size_t)bg * kc + j];
   const uint32_t it = lv.items[(size_t)bg * kc + j];
   if (id < 0 || (it & 0xC0000000u) != 0x80000000u) return;
   if (threadIdx.x == 0) {
-    const int way = (int)(it & 0x3FFFFFFFu);
-    const int gs = cv.seq_span_off[b] + id;
-    const int rr = lv.dir_rank[(size_t)g * spans_cap + gs];
-    const uint32_t bytes = (uint32_t)blob_dims(2, cv.span_len[gs], rr & 0xff, (rr >> 8) & 0xff).bytes;
+    const int gs = cv.seq_span_off[bg / Hkv] + id;
+    const uint32_t rr = (uint32_t)lv.dir_rank[(size_t)g * spans_cap + gs];
+    const uint32_t bytes = (uint32_t)blob_dims(2, (int)(rr >> 16), rr & 0xff, (rr >> 8) & 0xff).bytes;
     const uint8_t* src = host_arena + lv.dir_off[(size_t)g * spans_cap + gs];
-    uint8_t* dst = lv.slots + ((size_t)bg * ways + way) * slot_bytes;
+    uint8_t* dst = lv.slots + ((size_t)bg * ways + (it & 0x3FFFu)) * slot_bytes;
     mbar_init(&bar, 1);
     mbar_fence_init();
     uint32_t ph = 0u;
@@ -1396,7 +1495,6 @@ __global__ void __launch_bounds__(32) prefetch_kernel(CsrView cv, LayerView lv, 
       bulk_g2s(buf, src + o, n, &bar);
       mbar_wait(&bar, ph);
       ph ^= 1u;
-      fence_proxy_async();
       bulk_s2g(dst + o, buf, n);
       bulk_commit();
       bulk_wait_read_all();
@@ -1529,6 +1627,14 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
     P.trace_cap = left > 0 ? std::min(left, stride) : 0;
   }
   P.mode = mode; P.k = k; P.k_cap = c.k_cap; P.prefetch = std::max(c.prefetch, 0);
+  // Speculative prefetch (whole-step launches): the candidates of layer l are copied by the kernel of layer
+  // l + 1 (those of the last layer by layer 0 of the next step; sekv_api.cu covers the cases without one).
+  if (!((mode & FM_ROUTE) && (mode & FM_ATTN))) P.prefetch = 0;
+  if ((mode & FM_ROUTE) && (mode & FM_ATTN) && c.n_layers > 1 && c.prefetch > 0 && c.k_cap > 0) {
+    const int pl = (layer + c.n_layers - 1) % c.n_layers;       // layer 0 carries the last layer's copies of the previous step
+    P.pf_lv = layer_view(h, pl);
+    P.pf_plan_counts = (const int32_t*)ws(h, h->F.off_plan_counts) + (size_t)pl * c.max_seqs * c.n_kv_heads * 2;
+  }
   P.kc = std::max(c.k_cap, 1) + std::max(c.prefetch, 0);
   P.BG = h->n_seqs * c.n_kv_heads;
   P.Hq = c.n_q_heads; P.Hkv = c.n_kv_heads; P.dp = c.route_dim; P.ways = c.cache_ways;

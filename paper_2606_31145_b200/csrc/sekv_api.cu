@@ -93,7 +93,7 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   // >= 16 rows, one expanded span per ZOOM item at the finest)
   const int64_t attn_items = Hkv * (rcap / 16 + 2 * B + 2) + B * Hkv * kcap;
   F->max_chunks = (int)std::max<int64_t>(std::max(c.stage1_ctas, 1024) + B * Hkv, attn_items);
-  F->max_items = (int)(attn_items + 2 * B * Hq + B * Hkv + Hkv * (mcap / 8 + B + 1));
+  F->max_items = (int)(attn_items + 2 * B * Hq + B * Hkv * (1 + std::max(c.prefetch, 0)) + Hkv * (mcap / 8 + B + 1));
   const int G = c.n_q_heads / c.n_kv_heads;
   const int P2 = (kcap + kStage2SpansPerCta - 1) / kStage2SpansPerCta;
   F->off_partials1 = cv.take((size_t)F->max_chunks * G * kPartStride * 4);
@@ -386,6 +386,7 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
+  h->pending_prefetch = -1;
   h->n_items = 0; h->use_fused = false; h->fused_why = "no sequences built";
   h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
   h->span_len_host.clear();
@@ -556,6 +557,11 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
   const size_t first = std::min<size_t>((size_t)std::max(n_first, 0), pool_items.size());
   items.insert(items.end(), pool_items.begin(), pool_items.begin() + first);
   h->pool_end = (int)items.size();
+  // prefetch candidates of the previous layer of the step (copied by this layer's kernel; mostly no-ops)
+  if (c.k_cap > 0 && c.prefetch > 0 && c.n_layers > 1)
+    for (int b = 0; b < B; ++b)
+      for (int g = 0; g < Hkv; ++g)
+        for (int i = 0; i < c.prefetch; ++i) items.push_back(mk(IT_PREFETCH, b, g, i, 0, 0));
   items.insert(items.end(), zoom_items.begin(), zoom_items.end());
   items.insert(items.end(), coarse_items.begin(), coarse_items.end());
   items.insert(items.end(), pool_items.begin() + first, pool_items.end());
@@ -770,6 +776,10 @@ static cudaError_t decode_layer(sekv_handle* h, int layer, const void* q, const 
                                 void* out, float* lse) {
   cudaError_t e;
   if (h->use_fused) {     // caller-supplied zoom set: plan + attention + combine in the fused layer kernel
+    if (h->pending_prefetch == layer) {     // this layer's cache is about to be read: finish its prefetch copies first
+      if ((e = launch_prefetch(h, layer, h->main)) != cudaSuccess) return e;
+      h->pending_prefetch = -1;
+    }
     ProfScope ps(h, 6, h->main);
     return launch_fused(h, layer, FM_ATTN, q, nullptr, 0, nullptr, nullptr, (int32_t*)ids, (int32_t*)count, out, lse, h->main);
   }
@@ -808,7 +818,6 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
   const size_t qstride = (size_t)B * c.n_q_heads * kD * h->esize;
   const size_t ostride = (size_t)B * c.n_q_heads * kD * (c.out_dtype == SEKV_BF16 ? 2 : 4);
   const int kcap = std::max(c.k_cap, 1);
-  bool forked = false;
   for (int l = 0; l < c.n_layers; ++l) {
     const uint8_t* ql = (const uint8_t*)q + l * qstride;
     int32_t* ids = (int32_t*)(h->dev + h->F.off_ws_ids) + (size_t)l * c.max_seqs * c.n_kv_heads * kcap;
@@ -817,6 +826,11 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
     void* ol = (uint8_t*)out + l * ostride;
     float* ll = lse ? lse + (size_t)l * B * c.n_q_heads : nullptr;
     if (h->use_fused) {
+      if (c.n_layers == 1 && c.k_cap > 0 && c.prefetch > 0) {
+        // a one-layer model has no following layer kernel to carry the copies of the previous step's candidates
+        ProfScope ps(h, 7, h->main);
+        if ((e = launch_prefetch(h, 0, h->main)) != cudaSuccess) return e;
+      }
       {
         ProfScope ps(h, 6, h->main);
         if (c.k_cap > 0)
@@ -826,15 +840,6 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
           e = launch_fused(h, l, FM_ATTN, ql, nullptr, 0, nullptr, nullptr, nullptr, nullptr, ol, ll, h->main);
       }
       if (e != cudaSuccess) return e;
-      if (c.k_cap > 0 && c.prefetch > 0 && k >= 0) {
-        // speculative prefetch of the next-best spans of this layer on the side stream; it overlaps the
-        // following layers and is joined at the end of the step (this layer's cache is next read one step later)
-        if ((e = cudaEventRecord(h->ev_fork, h->main)) != cudaSuccess) return e;
-        if ((e = cudaStreamWaitEvent(h->side, h->ev_fork, 0)) != cudaSuccess) return e;
-        ProfScope ps(h, 7, h->side);
-        if ((e = launch_prefetch(h, l, h->side)) != cudaSuccess) return e;
-        forked = true;
-      }
       continue;
     }
     if (c.k_cap > 0) {
@@ -845,15 +850,10 @@ static cudaError_t enqueue_step(sekv_handle* h, const void* q, const float* tau,
     e = decode_layer(h, l, ql, ids, cnt, ol, ll);
     if (e != cudaSuccess) return e;
   }
-  if (forked) {
-    cudaError_t e;
-    if ((e = cudaEventRecord(h->ev_join, h->side)) != cudaSuccess) return e;
-    if ((e = cudaStreamWaitEvent(h->main, h->ev_join, 0)) != cudaSuccess) return e;
-  }
   return cudaSuccess;
 }
 
-sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out, float* lse) {
+static sekv_status decode_step_impl(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out, float* lse) {
   if (!h) return SEKV_INVALID_ARG;
   if (!h->segmented) return fail(h, SEKV_STATE, "no sequences built");
   for (int l = 0; l < h->cfg.n_layers; ++l)
@@ -883,7 +883,7 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   if (e != cudaSuccess || e2 != cudaSuccess) {
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
-    if (h->use_pdl) { h->use_pdl = false; return sekv_decode_step(h, q, tau, k, out, lse); }   // retry without the PDL edges
+    if (h->use_pdl) { h->use_pdl = false; return decode_step_impl(h, q, tau, k, out, lse); }   // retry without the PDL edges
     return cuda_fail(h, e != cudaSuccess ? e : e2, "decode_step graph capture");
   }
   GraphEntry ge{q, tau, k, out, lse, nullptr, nodes};
@@ -891,7 +891,7 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   cudaGraphDestroy(graph);
   if (e3 != cudaSuccess) {
     cudaGetLastError();
-    if (h->use_pdl) { h->use_pdl = false; return sekv_decode_step(h, q, tau, k, out, lse); }
+    if (h->use_pdl) { h->use_pdl = false; return decode_step_impl(h, q, tau, k, out, lse); }
     return cuda_fail(h, e3, "cudaGraphInstantiate");
   }
   if (h->graphs.size() >= 64) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
@@ -899,6 +899,14 @@ sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, in
   CK(h, cudaGraphLaunch(ge.exec, h->main));
   h->launches += nodes;
   return SEKV_OK;
+}
+
+sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out, float* lse) {
+  const sekv_status s = decode_step_impl(h, q, tau, k, out, lse);
+  // the last layer's prefetch candidates are copied by layer 0 of the next step (or before the next read of its cache)
+  if (s == SEKV_OK && h->use_fused && h->cfg.k_cap > 0 && h->cfg.prefetch > 0 && k >= 0)
+    h->pending_prefetch = h->cfg.n_layers - 1;
+  return s;
 }
 
 sekv_status sekv_last_zoom_ids(sekv_handle* h, int32_t layer, int32_t* ids, int32_t* count) {

@@ -138,13 +138,13 @@ enum StatIdx { ST_LAYER_STEPS = 0, ST_ZOOMED, ST_HITS, ST_MISSES, ST_H2D, ST_FAC
 // POOL, COARSE (L119-121), ZOOM (Eq. 8), COMBINE (L61).  The chain a1-a4 of a group (q' = W q, routing scores,
 // top-k, factor-cache plan) is not an item: a team of warps runs it at the start of the kernel (IT_SELECT is its
 // trace record).
-enum ItemKind { IT_QPROJ = 0, IT_ROUTE = 1, IT_SELECT = 2, IT_POOL = 3, IT_ZOOM = 4, IT_COARSE = 5, IT_COMBINE = 6 };
+enum ItemKind { IT_PREFETCH = 1, IT_SELECT = 2, IT_POOL = 3, IT_ZOOM = 4, IT_COARSE = 5, IT_COMBINE = 6 };
 enum FusedMode { FM_ROUTE = 1, FM_ATTN = 2 };   // FM_ATTN without FM_ROUTE: caller-supplied zoom set
 struct __align__(16) Item {   // 48 bytes: three 16-byte loads
   int32_t kind;        // ItemKind
   int32_t bg;          // b * H_kv + g
   int32_t a, b;        // COMBINE: a = head within the group, b = POOL + COARSE partials; POOL / COARSE: entry-row
-                       // range; ZOOM: plan-item range
+                       // range; ZOOM: a = descriptor index; PREFETCH: a = candidate index
   int32_t part;        // partial slot within the group (attention items)
   int32_t A;           // pool rows of the sequence
   int32_t row0;        // first entry row of the sequence
@@ -181,6 +181,8 @@ struct FusedParams {
   ZDescG* zdesc;               // [BG][kc] of this layer
   int32_t* ctrs;               // [0] work queue, [2] exited CTAs, then per group: early_done, -, attn_done, plan_flag
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
+  LayerView pf_lv;             // the previous layer of the step: its prefetch candidates are copied by this launch
+  const int32_t* pf_plan_counts;   // (null: nothing to copy)
   unsigned long long* stats;
   const uint8_t* host_arena;   // device alias of the pinned host factor store
   unsigned long long* trace;   // null, or 8 x u64 per item (sekv_set_trace)
@@ -289,6 +291,7 @@ struct sekv_handle {
   int num_sms;
   std::vector<GraphEntry> graphs;
   uint64_t launches;
+  int pending_prefetch;              // layer whose speculative prefetch copies have not been carried out yet (-1: none)
   // per-kernel-class CUDA-event timing (sekv_set_profiling)
   bool profiling;
   void* trace_buf; int64_t trace_cap;
@@ -332,8 +335,8 @@ cudaError_t launch_stage2(sekv_handle* h, int layer, const void* q, const int32_
 cudaError_t launch_combine(sekv_handle* h, int layer, void* out, float* lse, cudaStream_t s);
 cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, const float* tau, int k, float* logits,
                          float* alpha, int32_t* ids, int32_t* count, void* out, float* lse, cudaStream_t s);
-cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s);
 bool fused_geometry(const sekv_handle* h, FusedParams* P, std::string* why);
+cudaError_t launch_prefetch(sekv_handle* h, int layer, cudaStream_t s);
 cudaError_t fused_occupancy(const sekv_handle* h, int* ctas_per_sm);
 int fused_warps();
 
