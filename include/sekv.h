@@ -299,6 +299,8 @@ SEKV_API sekv_status sekv_get_kernel_times(sekv_handle* h, double* ms, uint64_t*
 SEKV_API sekv_status sekv_set_trace(sekv_handle* h, void* buf, int64_t capacity_items, int32_t* n_items);
 /* Number of stage-1 work chunks (CTAs) and partial slots per query head; HOST outs. */
 SEKV_API sekv_status sekv_get_schedule(const sekv_handle* h, int32_t* stage1_ctas, int32_t* parts_per_head);
+/* Number of CUDA graphs sekv_decode_step holds (one per distinct argument tuple; a replay adds none).  HOST out. */
+SEKV_API sekv_status sekv_graph_count(const sekv_handle* h, int32_t* count);
 /* Which kernels the built batch runs on.  *fused = 1: the persistent fused layer kernel (bf16 path, one launch
  * per layer-step); 0: the generic multi-kernel path, and *reason (a string owned by the handle, valid until the
  * next build / reset) says why -- fp32 storage, impl = 1, a sequence with too many spans for the team's shared

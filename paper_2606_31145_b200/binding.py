@@ -106,13 +106,14 @@ def _load() -> C.CDLL:
     lib.sekv_set_trace.argtypes = [VP, VP, I64, P(I32)]
     lib.sekv_build_sizes.argtypes = [P(sekv_config), I32, P(I64), VP, P(sekv_sizes), P(I32), P(I32)]
     lib.sekv_get_path.argtypes = [VP, P(I32), P(C.c_char_p)]
+    lib.sekv_graph_count.argtypes = [VP, P(I32)]
     lib.sekv_export_span_factors.argtypes = [VP, I32, I32, I32, I32, P(I32), P(I32), P(I32), VP, VP, VP, VP, VP, VP, P(I32)]
     for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
                  "sekv_last_zoom_ids",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
                  "sekv_static_bytes_per_layer", "sekv_get_schedule", "sekv_set_profiling",
-                 "sekv_get_kernel_times", "sekv_set_trace", "sekv_build_sizes", "sekv_get_path",
+                 "sekv_get_kernel_times", "sekv_set_trace", "sekv_build_sizes", "sekv_get_path", "sekv_graph_count",
                  "sekv_export_span_factors"):
         getattr(lib, name).restype = C.c_int
     return lib
@@ -356,6 +357,11 @@ class Sekv:
         cap = 0 if buf is None else buf.numel() * buf.element_size() // 64
         self._check(lib.sekv_set_trace(self._h, _ptr(buf), cap, C.byref(n)), "sekv_set_trace")
         self._trace_buf = buf
+        return int(n.value)
+
+    def sekv_graph_count(self) -> int:
+        n = C.c_int32(0)
+        self._check(lib.sekv_graph_count(self._h, C.byref(n)), "sekv_graph_count")
         return int(n.value)
 
     def sekv_get_path(self):

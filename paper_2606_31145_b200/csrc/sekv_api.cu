@@ -1028,6 +1028,12 @@ sekv_status sekv_set_trace(sekv_handle* h, void* buf, int64_t capacity_items, in
   return SEKV_OK;
 }
 
+sekv_status sekv_graph_count(const sekv_handle* h, int32_t* count) {
+  if (!h || !count) return SEKV_INVALID_ARG;
+  *count = (int32_t)h->graphs.size();
+  return SEKV_OK;
+}
+
 sekv_status sekv_get_path(const sekv_handle* h, int32_t* fused, const char** reason) {
   if (!h) return SEKV_INVALID_ARG;
   if (fused) *fused = h->use_fused ? 1 : 0;
