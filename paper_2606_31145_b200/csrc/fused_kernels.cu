@@ -173,9 +173,9 @@ __device__ __forceinline__ int team_excl_scan(const Team& T, int v, int* total) 
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void qproj_load(const FusedParams& P, int b, int g, int hl, int j0, int lane,
-                                           uint32_t (&qf)[4][4], uint4 (&w)[2][2][4]) {
+                                           uint32_t (&qf)[4][4], uint4 (&w)[2][2][4], bool with_q = true) {
   const int dp = P.dp, gid = lane >> 2, t4 = lane & 3;
-  if (j0 == 0) load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
+  if (j0 == 0 && with_q) load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
   const uint8_t* Wh = (const uint8_t*)P.lv.W + (size_t)(g * G + hl) * dp * (kD * 2) + t4 * 16;
 #pragma unroll
   for (int mt = 0; mt < 2; ++mt)
@@ -284,13 +284,15 @@ __device__ __forceinline__ void plan_init_scatter(const FusedParams& P, const Te
 template <int G>
 __device__ __forceinline__ void route_team(const FusedParams& P, Team& T, int bg, uint32_t* keys,
                                            float* sqp, const PlanTables& pt, int* span0_out, int* m_out,
-                                           unsigned long long* tm) {
+                                           bool pdl_wait, unsigned long long* tm) {
   const int b = bg / P.Hkv, g = bg % P.Hkv, dp = P.dp, lpr = dp >> 3, lane = T.lane;
-  // the query and W of this warp's head go first: they need nothing but the group index
+  // W of this warp's head goes first: it needs nothing but the group index.  With pdl_wait everything up to the
+  // query load (static tables only) runs BEFORE the programmatic-dependent-launch wait, i.e. in the tail of the
+  // previous layer's kernel; the query -- the one input that depends on the previous layer -- is read after it.
   uint32_t qf[4][4];
   uint4 wq[2][2][4];
   const int my_hl = T.tw;
-  if (my_hl < G) qproj_load<G>(P, b, g, my_hl, 0, lane, qf, wq);
+  if (my_hl < G) qproj_load<G>(P, b, g, my_hl, 0, lane, qf, wq, false);
   const int2 gi = __ldg(P.grp + bg);                             // first span and span count of the group's sequence
   const int span0 = gi.x, m = gi.y;
   *span0_out = span0; *m_out = m;
@@ -323,7 +325,9 @@ __device__ __forceinline__ void route_team(const FusedParams& P, Team& T, int bg
     uint32_t* hist = reinterpret_cast<uint32_t*>(T.tab + P.sm_hist);     // one histogram per radix pass of the select
     for (int i = T.tt; i < 4 * 256; i += T.ts) hist[i] = 0u;
   }
+  if (pdl_wait) asm volatile("griddepcontrol.wait;" ::: "memory");
   if (my_hl < G) {
+    load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, lane >> 2, lane & 3, qf);
     qproj_mma<G>(P, my_hl, 0, lane, qf, wq, sqp + my_hl * dp);
     for (int j0 = 32; j0 < dp; j0 += 32) {                       // d' = 64: the second half of W_h
       qproj_load<G>(P, b, g, my_hl, j0, lane, qf, wq);
@@ -434,6 +438,13 @@ __device__ __forceinline__ void route_team(const FusedParams& P, Team& T, int bg
   mark(tm, 0, T.tt);
 }
 
+// The zoom mask is all the COARSE items wait for.  It is published as self-validating (bits, step stamp) pairs --
+// 8-byte stores that the COARSE items poll; no flag, no fence.
+__device__ __forceinline__ void publish_mask(const FusedParams& P, const Team& T, const PlanTables& t, int bg, uint32_t epoch) {
+  uint2* gmask = P.zmask2 + (size_t)bg * P.mask_words;
+  for (int w = T.tt; w < P.mask_words; w += T.ts) gmask[w] = make_uint2(t.sh_mask[w], epoch);
+}
+
 // a4: residency plan of (b, g).  The device factor cache of a (layer, sequence, kv head) is `ways` slots with
 // a tag (span id) and a stamp (step of last use).  The first n_zoom entries of sh_ids are this step's zoom
 // set: resident ones are hits, the others are demand misses and take the least-recently-used slots not
@@ -444,7 +455,7 @@ __device__ __forceinline__ void route_team(const FusedParams& P, Team& T, int bg
 // expanded span for the ZOOM items, statistics.
 __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
                                           int m, int n_zoom, int n_cand, bool dedupe, uint32_t epoch,
-                                          unsigned long long* tm = nullptr) {
+                                          bool mask_done, unsigned long long* tm = nullptr) {
   const int g = bg % P.Hkv, ways = P.ways;
   int32_t* tags = P.lv.tags + (size_t)bg * ways;
   uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
@@ -499,12 +510,8 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   int n_need;
   team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1 to the team)
   n_need = min(n_need, ways);
-  // the zoom mask is all the COARSE items wait for: published before the misses are given slots, as
-  // self-validating (bits, step stamp) pairs -- 8-byte stores that the COARSE items poll, no flag, no fence
-  uint2* gmask = P.zmask2 + (size_t)bg * P.mask_words;
-  for (int w = T.tt; w < P.mask_words; w += T.ts) gmask[w] = make_uint2(t.sh_mask[w], epoch);
+  if (!mask_done) publish_mask(P, T, t, bg, epoch);
   if (T.tt == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
-  mark(tm, 3, T.tt);
   // victims: the n_need oldest ways not used by this step (ties to the lower way), by repeated extraction
   // of the minimum (stamp, way) -- only as many as this step has misses
   if (T.tw == 0) {
@@ -667,21 +674,27 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
 // The whole chain a1-a4 of group bg by the team.
 // ---------------------------------------------------------------------------------------------------
 template <int G>
-__device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int bg, uint32_t epoch,
+__device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int bg, uint32_t& epoch, bool pdl_wait,
                                             unsigned long long* tm) {
   const PlanTables t = plan_tables(P, T.tab);
   uint32_t* keys = reinterpret_cast<uint32_t*>(T.tab + P.sm_keys);
   float* sqp = reinterpret_cast<float*>(T.tab + P.sm_qp);
   int span0, m;
   if (P.mode & FM_ROUTE) {
-    route_team<G>(P, T, bg, keys, sqp, t, &span0, &m, tm);
+    route_team<G>(P, T, bg, keys, sqp, t, &span0, &m, pdl_wait, tm);
+    if (pdl_wait) epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
     int cnt, n_cand;
     select_team(P, T, t, keys, m, &cnt, &n_cand, tm);
     int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
     for (int j = T.tt; j < P.k_cap; j += T.ts) my_ids[j] = j < cnt ? t.sh_ids[j] : -1;
     if (T.tt == 0) P.count[bg] = cnt;
     if (P.mode & FM_ATTN) {
-      plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch, tm);
+      // the zoom set is known: its mask goes out first (routed ids are valid and distinct)
+      for (int j = T.tt; j < cnt; j += T.ts) atomicOr(&t.sh_mask[t.sh_ids[j] >> 5], 1u << (t.sh_ids[j] & 31));
+      team_bar(T);
+      publish_mask(P, T, t, bg, epoch);
+      mark(tm, 3, T.tt);
+      plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch, true, tm);
     }
   } else {
     // caller-supplied zoom set (sekv_decode_attn)
@@ -696,7 +709,7 @@ __device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int b
     team_bar(T);
     plan_init_scatter(P, T, t, m);
     team_bar(T);
-    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch);
+    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch, false);
   }
 }
 
@@ -751,49 +764,59 @@ __device__ __forceinline__ void ahead_resolve(const FusedParams& P, Ahead& a) {
   }
 }
 
-template <int G>
-__device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch,
-                                          Ahead& ah, unsigned long long* tm) {
-  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
-  const int gid = lane >> 2, t4 = lane & 3;
-  const int A = I.A, row_begin = I.a, row_end = I.b;
+// One 16-row K/V tile of a rows item -> ring stage t % kStages (cp.async).  Chunk idx = lane + 32 i of a 16 x 256-byte
+// tile is row r = 2 i + (lane >> 4), 16-byte chunk c = lane & 15: global offsets are contiguous and both swizzles are
+// per-lane constants plus compile-time terms in i.
+__device__ __forceinline__ void rows_fill(const FusedParams& P, const Item& I, uint8_t* region, int lane, int t) {
+  const int g = I.bg % P.Hkv, row_begin = I.a, row_end = I.b;
   const uint8_t* Kb = (const uint8_t*)P.lv.ent_k + ((size_t)g * P.ent_head_stride + (size_t)I.row0 * kD) * 2;
   const uint8_t* Vb = (const uint8_t*)P.lv.ent_v + ((size_t)g * P.ent_head_stride + (size_t)I.row0 * kD) * 2;
-  const float scale2 = rsqrtf((float)kD) * kLog2e;
-  const int ntiles = (row_end - row_begin + 15) >> 4;
-
-  // chunk idx = lane + 32 i of a 16 x 256-byte tile is row r = 2 i + (lane >> 4), 16-byte chunk c = lane & 15:
-  // global offsets are contiguous and both swizzles are per-lane constants plus compile-time terms in i
   const int lr = lane >> 4, lc = lane & 15;
   const uint32_t dk0 = (uint32_t)(lr * 256 + ((lc ^ (lr << 2)) << 4));
   const uint32_t dv0 = (uint32_t)(lr * 256);
   const uint32_t lcx = (uint32_t)(lc ^ lr);
-  auto fill = [&](int t) {
-    uint8_t* Ks = region + (t % kStages) * kStageBytes;
-    uint8_t* Vs = Ks + 16 * kD * 2;
-    const int r0 = row_begin + t * 16;
-    if (r0 + 16 <= row_end) {                                   // full tile: no clamping
-      const size_t src = (size_t)r0 * (kD * 2) + lane * 16;
+  uint8_t* Ks = region + (t % kStages) * kStageBytes;
+  uint8_t* Vs = Ks + 16 * kD * 2;
+  const int r0 = row_begin + t * 16;
+  if (r0 + 16 <= row_end) {                                   // full tile: no clamping
+    const size_t src = (size_t)r0 * (kD * 2) + lane * 16;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        cp_async16(Ks + dk0 + 512 * i, Kb + src + 512 * i);
-        cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src + 512 * i);
-      }
-    } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int r = 2 * i + lr;
-        const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + lc * 16;
-        cp_async16(Ks + dk0 + 512 * i, Kb + src);
-        cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src);
-      }
+    for (int i = 0; i < 8; ++i) {
+      cp_async16(Ks + dk0 + 512 * i, Kb + src + 512 * i);
+      cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src + 512 * i);
     }
-  };
+  } else {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int r = 2 * i + lr;
+      const size_t src = (size_t)min(r0 + r, row_end - 1) * (kD * 2) + lc * 16;
+      cp_async16(Ks + dk0 + 512 * i, Kb + src);
+      cp_async16(Vs + dv0 + 512 * i + ((lcx ^ ((2 * i) & 7)) << 4), Vb + src);
+    }
+  }
+}
+// the first kStages tiles of a rows item (static tables: may run before the programmatic-dependent-launch wait)
+__device__ __forceinline__ void rows_prefill(const FusedParams& P, const Item& I, uint8_t* region, int lane) {
+  const int ntiles = (I.b - I.a + 15) >> 4;
 #pragma unroll
   for (int t = 0; t < kStages; ++t) {
-    if (t < ntiles) fill(t);
+    if (t < ntiles) rows_fill(P, I, region, lane, t);
     cp_async_commit();
   }
+}
+
+template <int G>
+__device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch,
+                                          Ahead& ah, bool prefilled, unsigned long long* tm) {
+  const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
+  const int gid = lane >> 2, t4 = lane & 3;
+  const int A = I.A, row_begin = I.a, row_end = I.b;
+  const float scale2 = rsqrtf((float)kD) * kLog2e;
+  const int ntiles = (row_end - row_begin + 15) >> 4;
+  if (!prefilled) rows_prefill(P, I, region, lane);
+  uint32_t qf[4][4];                                           // (before the COARSE item's poll: its latency overlaps the wait)
+  load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
+
   // biases of a COARSE item: lane L holds rows row_begin + L and row_begin + 32 + L (ln|S| in the base-2 domain;
   // -inf for an expanded span, whose coarse entry is replaced by its tokens, and for rows past the item)
   float bias_reg[2] = {0.f, 0.f};
@@ -823,8 +846,6 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
     __syncwarp();
     mark(tm, 0, lane);
   }
-  uint32_t qf[4][4];
-  load_q_frags(P.q + ((size_t)b * P.Hq + (size_t)g * G) * kD, G, gid, t4, qf);
   float m_run = -INFINITY, l_run = 0.f;
   float of[8][4];
 #pragma unroll
@@ -901,7 +922,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
       mma16816_full(of[md], a0, a1, a2, a3, b0l, b1l);
     }
     __syncwarp();                                      // every lane is done with this stage
-    if (t + kStages < ntiles) fill(t + kStages);
+    if (t + kStages < ntiles) rows_fill(P, I, region, lane, t + kStages);
     cp_async_commit();
     if (t == 0) ahead_resolve(P, ah);
   }
@@ -965,7 +986,8 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
                                           bool hdr_smem, int len, int nks, int nvs, uint8_t* region, uint32_t cap_bytes,
                                           uint64_t* bar, uint32_t& phase, int lane,
                                           const uint32_t (&qf)[4][4], float& M, float& L, float (&of)[8][4],
-                                          uint8_t* wb, bool wb_regs, unsigned long long* tm) {
+                                          uint8_t* wb, bool wb_regs, uint64_t* hbar, uint32_t* hphase, uint32_t hdr_bytes,
+                                          unsigned long long* tm) {
   // blob: where the chunk windows come from (cache slot, or the pinned-host copy of a demand miss); hdr: the header
   // (= blob, or a copy staged in shared memory); region / cap_bytes: where the windows go.
   // wb: null, or the cache slot a demand miss is kept in: the chunk windows are written to it by bulk copies out
@@ -983,6 +1005,11 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
   const int win = max(1, min(nchunks, fit >= CH ? fit / CH * CH : fit));
   const float scale2 = rsqrtf((float)kD) * kLog2e;
   region_fetch_start(region, blob + off_ch, (uint32_t)min(win, nchunks) * chunk_bytes, bar, lane);
+  if (hbar != nullptr) {                               // demand miss: the staged header (in flight together with the window)
+    mbar_wait(hbar, *hphase);
+    *hphase ^= 1u;
+    if (wb && lane == 0) { bulk_s2g(wb, hdr, hdr_bytes); bulk_commit(); }
+  }
   // V_V is needed last: pull it towards L2 now
   if (NK != 1 && !hdr_smem)
     for (int i = lane; i < nvs * 32; i += 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(hdr + off_vv + (size_t)i * 128));
@@ -1172,7 +1199,7 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
-                                          uint32_t& phase, int lane, uint32_t epoch, unsigned long long* tm) {
+                                          uint32_t& phase, uint32_t& phase1, int lane, uint32_t epoch, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
   uint32_t qf[4][4];
@@ -1197,14 +1224,21 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
     uint8_t* cbase = region;
     uint32_t cap = (uint32_t)P.region_bytes;
     bool hdr_smem = false, wb_regs = wb != nullptr;
+    uint64_t* hbar = nullptr;
     if (miss && hdr_bytes + chunk_bytes <= (uint32_t)P.region_bytes) {
-      region_fetch(region, blob, hdr_bytes, bar, phase, lane);
-      if (wb && lane == 0) { bulk_s2g(wb, region, hdr_bytes); bulk_commit(); }
+      __syncwarp();
+      if (lane == 0) {                                 // header -> front of the region, on the warp's second barrier
+        mbar_arrive_expect_tx(bar + 1, hdr_bytes);
+        bulk_g2s(region, blob, hdr_bytes, bar + 1);
+      }
+      hbar = bar + 1;
       hdr = region; hdr_smem = true; wb_regs = false;
       cbase = region + hdr_bytes; cap = (uint32_t)P.region_bytes - hdr_bytes;
     }
-    if (nks <= 1 && nvs <= 1) zoom_span<G, 1>(P, blob, hdr, hdr_smem, len, 1, 1, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, tm);
-    else zoom_span<G, 4>(P, blob, hdr, hdr_smem, len, nks, nvs, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, tm);
+    if (nks <= 1 && nvs <= 1)
+      zoom_span<G, 1>(P, blob, hdr, hdr_smem, len, 1, 1, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, hbar, &phase1, hdr_bytes, tm);
+    else
+      zoom_span<G, 4>(P, blob, hdr, hdr_smem, len, nks, nvs, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, hbar, &phase1, hdr_bytes, tm);
   } else {
 #pragma unroll
     for (int n = 0; n < 8; ++n) { of[n][0] = of[n][1] = of[n][2] = of[n][3] = 0.f; }
@@ -1347,31 +1381,45 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
     mbar_fence_init();
   }
   __syncwarp();
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  const uint32_t epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
-  uint32_t phase = 0u;
+  uint32_t phase = 0u, phase1 = 0u;                   // parities of the warp's two barriers
   unsigned long long* tm = P.trace ? &tmid_s[warp * 4] : nullptr;
 
   // The chain of group bg runs on the team (warps 0 .. team_warps-1) of CTA bg % grid, starting at t = 0.  All
   // other warps take their first work item statically (no claim latency at the start) and claim from there on.
+  // Whatever needs only static tables runs BEFORE the dependency wait, i.e. while the previous layer's kernel
+  // drains: the first K/V tiles of a POOL item, and (P.hoist) the chain's tables, routing blocks and W.  The
+  // query -- the one input that depends on the previous layer -- is read after the wait.
   const int ntw = P.team_warps;
   const int n_chain_cta = P.has_chain ? min(P.BG, (int)gridDim.x) : 0;
   const bool chain_cta = (int)blockIdx.x < n_chain_cta;
-  int idx;
-  if (chain_cta && warp < ntw) {
+  const bool is_team = chain_cta && warp < ntw;
+  uint32_t epoch = 0u;
+  int idx = -1;
+  Item first;
+  bool prefilled = false;
+  if (!is_team) {
+    const int b = (int)blockIdx.x;
+    idx = chain_cta ? b * (nw - ntw) + (warp - ntw) : n_chain_cta * (nw - ntw) + (b - n_chain_cta) * nw + warp;
+    if (idx < P.main_end) {
+      first = load_item(P.items + idx);
+      if (first.kind == IT_POOL) { rows_prefill(P, first, region, lane); prefilled = true; }
+    }
+  }
+  if (!is_team || !P.hoist) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
+  }
+  if (is_team) {
     Team T;
     T.tt = tid; T.ts = ntw * 32; T.lane = lane; T.tw = warp; T.ntw = ntw; T.scratch = team_scratch;
     T.tab = dsm; T.stage = dsm + P.sm_stage + (size_t)warp * P.stage_bytes;
     T.bars = &bars[warp][0]; T.ph[0] = 0u; T.ph[1] = 0u;
+    bool pdl_wait = P.hoist != 0;
     for (int bg = (int)blockIdx.x; bg < P.BG; bg += (int)gridDim.x) {
       unsigned long long t0 = 0ull;
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
-      chain_group<G>(P, T, bg, epoch, tm);
-#ifdef SEKV_CHAIN_TWICE
-      team_bar(T);
-      if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
-      chain_group<G>(P, T, bg, epoch, tm);
-#endif
+      chain_group<G>(P, T, bg, epoch, pdl_wait, tm);
+      pdl_wait = false;
       const int rec = P.main_end + bg;                         // trace record after the queue items
       if (P.trace && tid == 0 && rec < P.trace_cap) {
         unsigned long long* r = P.trace + 8 * (size_t)rec;
@@ -1382,11 +1430,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
       }
       team_bar(T);                                             // the tables are free for the next group
     }
-    phase = T.ph[0];                                           // the items go on with barrier 0 of this warp
-    idx = -1;
-  } else {
-    const int b = (int)blockIdx.x;
-    idx = chain_cta ? b * (nw - ntw) + (warp - ntw) : n_chain_cta * (nw - ntw) + (b - n_chain_cta) * nw + warp;
+    phase = T.ph[0]; phase1 = T.ph[1];                         // the items go on with this warp's barriers
   }
   const int n_static = n_chain_cta * (nw - ntw) + ((int)gridDim.x - n_chain_cta) * nw;
   auto claim = [&]() -> int {
@@ -1394,11 +1438,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
     if (lane == 0) i = n_static + atomicAdd(P.ctrs, 1);
     return __shfl_sync(0xffffffffu, i, 0);
   };
-  if (idx < 0) idx = claim();
+  if (is_team) idx = claim();
   if (idx < P.main_end) {
     // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular).  Any other
     // item is claimed when the warp is free to run it, so it never waits behind a slow item.
-    Item cur = load_item(P.items + idx);
+    Item cur = is_team ? load_item(P.items + idx) : first;
     for (;;) {
       Ahead ah;
       ah.on = cur.kind == IT_POOL; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
@@ -1408,8 +1452,8 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
       switch (cur.kind) {
         case IT_POOL:
-        case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ah, tm); break;
-        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, lane, epoch, tm); break;
+        case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ah, prefilled, tm); prefilled = false; break;
+        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, phase1, lane, epoch, tm); break;
         case IT_PREFETCH: if (P.pf_plan_counts != nullptr) prefetch_item(P, cur, region, bar, phase, lane); break;
         default: combine_item(P, cur, region, bar, phase, lane, tm); break;
       }
@@ -1647,6 +1691,9 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.zmask2 = (uint2*)ws(h, h->F.off_zmask2) + (size_t)layer * c.max_seqs * c.n_kv_heads * h->mask_words;
   // the chain (a1-a4) runs whenever there is routing to do or a zoom set to plan
   P.has_chain = ((mode & FM_ROUTE) || c.k_cap > 0) ? 1 : 0;
+  // whole-step launches of a model with more than one layer: the previous kernel on the stream is another layer's
+  // (it writes none of this layer's tables), so the chain's static part may run before the dependency wait
+  P.hoist = ((mode & FM_ROUTE) && (mode & FM_ATTN) && c.n_layers > 1) ? 1 : 0;
   if ((mode & FM_ROUTE) && (mode & FM_ATTN)) {                  // whole-step launches run the layers in order
     const LayerView nv = layer_view(h, (layer + 1) % c.n_layers);
     P.next_W = (const uint8_t*)nv.W;

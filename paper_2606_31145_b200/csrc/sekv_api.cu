@@ -562,8 +562,14 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
     for (int b = 0; b < B; ++b)
       for (int g = 0; g < Hkv; ++g)
         for (int i = 0; i < c.prefetch; ++i) items.push_back(mk(IT_PREFETCH, b, g, i, 0, 0));
-  items.insert(items.end(), zoom_items.begin(), zoom_items.end());
+  // ZOOM positions 0 and 1 of every group first (the plan puts demand misses there: their blobs cross PCIe), then
+  // the COARSE items (two tiles each, in flight while the item waits for the zoom mask; ~1 us of work after it),
+  // then the other ZOOM items
+  std::vector<Item> zoom_early, zoom_late;
+  for (const Item& it : zoom_items) (it.a < 2 ? zoom_early : zoom_late).push_back(it);
+  items.insert(items.end(), zoom_early.begin(), zoom_early.end());
   items.insert(items.end(), coarse_items.begin(), coarse_items.end());
+  items.insert(items.end(), zoom_late.begin(), zoom_late.end());
   items.insert(items.end(), pool_items.begin() + first, pool_items.end());
   for (int b = 0; b < B; ++b)
     for (int g = 0; g < Hkv; ++g)

@@ -196,6 +196,7 @@ struct FusedParams {
   int32_t mode, k, k_cap, prefetch, kc, BG;
   int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, out_bf16;
   int32_t region_bytes;                          // per-warp shared-memory region
+  int32_t hoist;                                 // the chain's static part may run before the PDL wait
   int32_t team_warps, has_chain;                 // warps 0 .. team_warps-1 of CTA bg % grid run the chain of group bg
   int32_t route_spans, route_bufs;               // spans per routing block, staging buffers per team warp (1 or 2)
   int32_t sm_stage, stage_bytes;                 // staging buffers: dsm + sm_stage + warp * stage_bytes
