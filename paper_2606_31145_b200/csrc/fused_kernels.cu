@@ -105,9 +105,26 @@ __device__ __forceinline__ float hdr_ldf(const uint8_t* p, bool in_smem) {
   return in_smem ? *reinterpret_cast<const float*>(p) : __ldcg(reinterpret_cast<const float*>(p));
 }
 
-// per-group counters inside P.ctrs
-__device__ __forceinline__ int32_t* grp_ctr(const FusedParams& P, int bg, int which) { return P.ctrs + 4 + 4 * bg + which; }
-enum { C_EARLY = 0, C_ATTN = 2 };   // C_EARLY: POOL + COARSE items done, C_ATTN: every attention item done
+// Counters of a launch (one of two sets per layer, alternating with the layer's launch sequence number: the set a
+// launch uses was zeroed during the previous launch of the layer, so nothing is re-armed in the kernel's tail):
+// [0] work queue, [1] warps that have read the sequence number, then one word per group: attention items done,
+// POOL + COARSE items in the low 16 bits (kEarlyOne), all kinds in the high 16 bits (kAttnOne).
+__device__ __forceinline__ int32_t* grp_ctr(int32_t* ctrs, int bg) { return ctrs + 4 + 4 * bg; }
+constexpr int kEarlyOne = 0x00010001, kAttnOne = 0x00010000;
+// spin (lane 0) until the 16-bit field of the group's counter reaches `target`
+__device__ __forceinline__ void wait_field(const int32_t* c, int shift, int target, int lane, unsigned long long* t_mid = nullptr) {
+  if (lane == 0) {
+    int v;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
+      if (((v >> shift) & 0xFFFF) >= target) break;
+      __nanosleep(64);
+    }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+    if (t_mid) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(*t_mid));
+  }
+  __syncwarp();
+}
 
 // spin (lane 0) until the counter reaches `target`
 // (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
@@ -807,7 +824,7 @@ __device__ __forceinline__ void rows_prefill(const FusedParams& P, const Item& I
 
 template <int G>
 __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, uint8_t* region, int lane, uint32_t epoch,
-                                          Ahead& ah, bool prefilled, unsigned long long* tm) {
+                                          int32_t* ctrs, Ahead& ah, bool prefilled, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
   const int A = I.A, row_begin = I.a, row_end = I.b;
@@ -930,10 +947,7 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   ahead_resolve(P, ah);
   store_partial<G>(P, I, lane, m_run, l_run, of);
   __syncwarp();
-  if (lane == 0) {
-    red_add_release(grp_ctr(P, bg, C_EARLY), 1);
-    red_add_release(grp_ctr(P, bg, C_ATTN), 1);
-  }
+  if (lane == 0) red_add_release(grp_ctr(ctrs, bg), kEarlyOne);
 }
 
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
@@ -1199,7 +1213,8 @@ __device__ __forceinline__ void zoom_span(const FusedParams& P, const uint8_t* _
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
-                                          uint32_t& phase, uint32_t& phase1, int lane, uint32_t epoch, unsigned long long* tm) {
+                                          uint32_t& phase, uint32_t& phase1, int lane, uint32_t epoch, int32_t* ctrs,
+                                          unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv;
   const int gid = lane >> 2, t4 = lane & 3;
   uint32_t qf[4][4];
@@ -1247,7 +1262,8 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
   Item Ij = I;                                                   // the partial of list index j goes to slot j
   Ij.part = I.part - I.a + (int)((d.way_miss >> 14) & 0xFFFFu);
   store_partial<G>(P, Ij, lane, M, L, of);
-  signal_ctr(grp_ctr(P, bg, C_ATTN), lane);
+  __syncwarp();
+  if (lane == 0) red_add_release(grp_ctr(ctrs, bg), kAttnOne);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -1293,7 +1309,7 @@ __device__ __forceinline__ void prefetch_item(const FusedParams& P, const Item& 
 // contiguous; they move into the warp's region by bulk copies and are reduced from shared memory.
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I, uint8_t* region, uint64_t* bar,
-                                             uint32_t& phase, int lane, unsigned long long* tm) {
+                                             uint32_t& phase, int lane, int32_t* ctrs, unsigned long long* tm) {
   const int bg = I.bg, b = bg / P.Hkv, g = bg % P.Hkv, hl = I.a, np = I.np;
   const int G = P.Hq / P.Hkv;
   const float* src = P.partials + ((size_t)I.pbase + (size_t)hl * np) * kPartStride;
@@ -1304,10 +1320,10 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
   // two phases: the POOL and COARSE partials (slots [0, I.b)) are complete long before the expanded spans
   // are; they are merged while those are still running, so only the ZOOM partials remain for the tail
   const int n_pool = I.b;
-  wait_ctr(grp_ctr(P, bg, C_EARLY), n_pool, lane, nullptr);
+  wait_field(grp_ctr(ctrs, bg), 0, n_pool, lane, nullptr);
   bool second = false;
   for (int p0 = 0; p0 < np; p0 += cap) {
-    if (!second && p0 >= n_pool) { wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm); second = true; }
+    if (!second && p0 >= n_pool) { wait_field(grp_ctr(ctrs, bg), 16, np, lane, tm); second = true; }
     const int n = min(cap, (second ? np : n_pool) - p0);
     region_fetch(region, src + (size_t)p0 * kPartStride, (uint32_t)(n * kPartStride * 4), bar, phase, lane);
     float mc = -INFINITY;
@@ -1336,7 +1352,7 @@ __device__ __forceinline__ void combine_item(const FusedParams& P, const Item& I
     M = Mn;
     if (!second && p0 + n >= n_pool) { p0 = n_pool - cap; }     // next round starts at the first non-POOL partial
   }
-  if (!second) wait_ctr(grp_ctr(P, bg, C_ATTN), np, lane, tm);  // (no ZOOM partials at all)
+  if (!second) wait_field(grp_ctr(ctrs, bg), 16, np, lane, tm);  // (no ZOOM partials at all)
   const float inv = L > 0.f ? 1.f / L : 0.f;
   const size_t oi = ((size_t)b * P.Hq + (size_t)g * G + hl) * kD + 4 * lane;
   if (P.out_bf16) {
@@ -1365,7 +1381,6 @@ template <int G>
 __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __grid_constant__ FusedParams P) {
   extern __shared__ __align__(128) uint8_t dsm[];
   __shared__ uint64_t bars[kFusedWarps][2];
-  __shared__ int last_flag;
   __shared__ unsigned long long tmid_s[kFusedWarps * 4];
   __shared__ int team_scratch[32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
@@ -1409,6 +1424,10 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
     asm volatile("griddepcontrol.wait;" ::: "memory");
     epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
   }
+  // The layer's launch sequence number picks the counter set.  (It is only written by launches of this layer: a
+  // hoisted team, which has not waited yet, follows another layer's kernel and reads a settled value.)
+  const uint32_t seq = *reinterpret_cast<volatile const uint32_t*>(P.ctrs);
+  int32_t* ctrs = P.ctrs + 4 + (seq & 1u) * P.ctrs_set;
   if (is_team) {
     Team T;
     T.tt = tid; T.ts = ntw * 32; T.lane = lane; T.tw = warp; T.ntw = ntw; T.scratch = team_scratch;
@@ -1432,30 +1451,38 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
     }
     phase = T.ph[0]; phase1 = T.ph[1];                         // the items go on with this warp's barriers
   }
+  // this warp has read the layer's sequence number and step stamp (both are advanced by one thread at the end of
+  // the launch, once every warp of the grid has said so here)
+  __syncwarp();
+  if (lane == 0) asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(ctrs + 1), "r"(1) : "memory");
+  if (blockIdx.x == gridDim.x - 1) {                             // the other set: for the next launch of this layer
+    int32_t* other = P.ctrs + 4 + ((seq + 1u) & 1u) * P.ctrs_set;
+    for (int i = tid; i < P.ctrs_set; i += blockDim.x) other[i] = 0;
+  }
   const int n_static = n_chain_cta * (nw - ntw) + ((int)gridDim.x - n_chain_cta) * nw;
   auto claim = [&]() -> int {
     int i = 0;
-    if (lane == 0) i = n_static + atomicAdd(P.ctrs, 1);
+    if (lane == 0) i = n_static + atomicAdd(ctrs, 1);
     return __shfl_sync(0xffffffffu, i, 0);
   };
   if (is_team) idx = claim();
   if (idx < P.main_end) {
-    // Claims run ahead only through POOL items (no dependencies, nobody waits on one in particular).  Any other
-    // item is claimed when the warp is free to run it, so it never waits behind a slow item.
+    // Claims run ahead only through POOL and COARSE items (short or dependency-free: the claimed item does not wait
+    // long behind them).  Any other item is claimed when the warp is free to run it.
     Item cur = is_team ? load_item(P.items + idx) : first;
     for (;;) {
       Ahead ah;
-      ah.on = cur.kind == IT_POOL; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
-      if (ah.on && lane == 0) ah.pending = atomicAdd(P.ctrs, 1);
+      ah.on = cur.kind == IT_POOL || cur.kind == IT_COARSE; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
+      if (ah.on && lane == 0) ah.pending = atomicAdd(ctrs, 1);
       unsigned long long t0 = 0ull;
       const int cur_idx = idx;
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
       switch (cur.kind) {
         case IT_POOL:
-        case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ah, prefilled, tm); prefilled = false; break;
-        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, phase1, lane, epoch, tm); break;
+        case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ctrs, ah, prefilled, tm); prefilled = false; break;
+        case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, phase1, lane, epoch, ctrs, tm); break;
         case IT_PREFETCH: if (P.pf_plan_counts != nullptr) prefetch_item(P, cur, region, bar, phase, lane); break;
-        default: combine_item(P, cur, region, bar, phase, lane, tm); break;
+        default: combine_item(P, cur, region, bar, phase, lane, ctrs, tm); break;
       }
       if (P.trace && lane == 0 && cur_idx < P.trace_cap) {
         unsigned int smid;
@@ -1489,18 +1516,17 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
       asm volatile("prefetch.global.L2 [%0];" ::"l"(P.next_route + h * P.route_head_stride * 2 + (li << 7)));
     }
   }
-  // last CTA out re-arms the queue and the counters and advances the layer's step stamp
-  __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    const int old = atomicAdd(P.ctrs + 2, 1);
-    last_flag = (old == (int)gridDim.x - 1);
-  }
-  __syncthreads();
-  if (last_flag) {
-    __threadfence();
-    for (int i = tid; i < 4 + 4 * P.BG; i += blockDim.x) P.ctrs[i] = 0;
-    if (tid == 0 && (P.mode & FM_ATTN)) {
+  // Nothing is re-armed here and no CTA waits for another one on the way out.  One thread advances the layer's
+  // sequence number and step stamp once every CTA has read them (they did at their start; the count is a check).
+  if (blockIdx.x == 0 && tid == 0) {
+    int v;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ctrs + 1) : "memory");
+      if (v >= (int)(gridDim.x * (blockDim.x >> 5))) break;
+      __nanosleep(64);
+    }
+    *reinterpret_cast<volatile uint32_t*>(P.ctrs) = seq + 1u;
+    if (P.mode & FM_ATTN) {
       *P.lv.layer_step = epoch;
       atomicAdd(&P.stats[ST_LAYER_STEPS], 1ull);
     }
@@ -1661,6 +1687,7 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.partials = (float*)ws(h, h->F.off_partials1);
   P.zdesc = (ZDescG*)ws(h, h->F.off_zdesc) + (size_t)layer * c.max_seqs * c.n_kv_heads * (std::max(c.k_cap, 1) + std::max(c.prefetch, 0));
   P.ctrs = (int32_t*)ws(h, h->F.off_ctrs) + (size_t)layer * h->F.ctrs_per_layer;
+  P.ctrs_set = (h->F.ctrs_per_layer - 4) / 2;
   P.plan_counts = (int32_t*)ws(h, h->F.off_plan_counts) + (size_t)layer * c.max_seqs * c.n_kv_heads * 2;
   P.stats = (unsigned long long*)ws(h, h->F.off_stats);
   P.host_arena = h->host_dev;

@@ -110,7 +110,7 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   F->off_items_sched = cv.take((size_t)F->max_items * sizeof(Item));
   F->off_bg_part = cv.take((size_t)(B * Hkv + 1) * 8);          // int2 per group: first span, span count
   F->off_bg_route = cv.take((size_t)(B * Hkv) * 4);
-  F->ctrs_per_layer = (int)(4 + 4 * B * Hkv);
+  F->ctrs_per_layer = (int)(4 + 2 * (4 + 4 * B * Hkv));       // sequence number + two counter sets
   F->off_zdesc = cv.take((size_t)NL * B * Hkv * kc * sizeof(ZDescG));
   F->off_zmask2 = cv.take((size_t)NL * B * Hkv * F->mask_words * 8);
   F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);

@@ -179,7 +179,8 @@ struct FusedParams {
   const int2* grp;             // [BG] first span and span count of the group's sequence
   float* partials;             // records [pbase + hl * np + part][kPartStride]
   ZDescG* zdesc;               // [BG][kc] of this layer
-  int32_t* ctrs;               // [0] work queue, [2] exited CTAs, then per group: early_done, -, attn_done, plan_flag
+  int32_t* ctrs;               // [0] launch sequence number of the layer, then two counter sets (fused_kernels.cu)
+  int32_t ctrs_set;            // ints per set
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
   LayerView pf_lv;             // the previous layer of the step: its prefetch candidates are copied by this launch
   const int32_t* pf_plan_counts;   // (null: nothing to copy)
