@@ -24,8 +24,32 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "sekv_decode_attn_us_per_layer_step_128k"
-NCU_DRAM_BYTES_PER_LAUNCH = 122.9e6   # 118.1 MB read + 4.9 MB written (algorithmic: 108.6 MB)
 UNIT = "us/layer-step"
+NCU_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+KERNEL_SOURCES = ("fused_kernels.cu", "mma_common.cuh", "sekv_internal.cuh")
+
+
+def kernel_sha256() -> str:
+    """Digest of the sources of the layer kernel: the ncu traffic figure is only quoted for the kernel it was
+    captured on (profiles/r02_ncu_traffic.json records this digest)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2606_31145_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def ncu_traffic_per_launch():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the layer kernel from the tracked ncu capture,
+    or None when the kernel sources have changed since (a stale figure is not quoted)."""
+    try:
+        d = json.load(open(NCU_TRAFFIC_JSON))
+    except Exception:
+        return None, "no tracked ncu capture"
+    if d.get("kernel_sha256") != kernel_sha256():
+        return None, "stale: kernel sources changed since the capture at %s" % d.get("commit", "?")
+    return float(d["dram_bytes_per_launch"]), "profiles/r02_ncu_traffic.json (captured at %s)" % d.get("commit", "?")
 
 
 def parse():
@@ -49,7 +73,9 @@ def parse():
     ap.add_argument("--item-rows", type=int, default=0)
     ap.add_argument("--zoom-spans", type=int, default=0)
     ap.add_argument("--profile-steps", type=int, default=4)
-    ap.add_argument("--e2e-steps", type=int, default=8)
+    ap.add_argument("--e2e-steps", type=int, default=24)
+    ap.add_argument("--sweep-steps", type=int, default=10, help="timed steps per rho of the sweep (0 = no sweep)")
+    ap.add_argument("--oracle-worker", default="", help=argparse.SUPPRESS)
     return ap.parse_args()
 
 
@@ -82,11 +108,25 @@ def measured_peaks():
 # ---------------------------------------------------------------------------------------------
 # the oracle on the host cores: reference arm and cpu_baseline leg
 # ---------------------------------------------------------------------------------------------
-def oracle_sample(spec, steps: int, warmup: int, rho: float):
+_ORACLE_STATE = {}
+
+
+def _oracle_head(arg):
+    """Pool worker (forked after the tables were built: shares them copy-on-write): the oracle's mixed attention
+    for one query head."""
+    h, q, ids = arg
+    st = _ORACLE_STATE
+    out, lse = st["O"].decode_attn(q, st["T"], ids, heads=[h])
+    return h, out[h], lse[h]
+
+
+def oracle_sample(spec, steps: int, warmup: int, rho: float, all_cores: bool = False):
     """Time the oracle (as it stands) on a bounded sample of the workload: ONE sequence of the batch at
     ONE layer -- its own prefill-time construction from the seeded generator (untimed), then per
-    step routing + mixed-resolution attention for all query heads (timed).  Returns seconds per
-    (sequence, layer-step) and the sample description."""
+    step routing + mixed-resolution attention for all query heads (timed), on one thread and, with
+    all_cores, with one forked process per query head over all host cores.  Returns a dict with
+    seconds per (sequence, layer-step) for both and the sample description."""
+    import multiprocessing as mp
     import numpy as np
     import torch
     from oracle import sekv_oracle as O
@@ -110,22 +150,51 @@ def oracle_sample(spec, steps: int, warmup: int, rho: float):
                        dtype=one.dtype, prefactored=pre)
     del K, V, pre
     q = make_queries(one, 0, "cpu")
-    times = []
+    qs = []
     for i in range(warmup + steps):
-        qn = f64(q)[0, 0]
+        qs.append(f64(q)[0, 0])
+        q = next_queries_ar1(one, q, i + 1, rho)
+    times = []
+    for i, qn in enumerate(qs):
         t0 = time.perf_counter()
         R = O.route(qn, T.W, T.route_K, T.seg.span_len, one.n_kv_heads, one.top_k)
-        O.decode_attn(qn, T, R.ids)
+        ref, _ = O.decode_attn(qn, T, R.ids)
         dt = time.perf_counter() - t0
         if i >= warmup:
             times.append(dt)
-        q = next_queries_ar1(one, q, i + 1, rho)
+    res = {"sec_1": float(np.mean(times)), "cores_all": 1, "sec_all": None}
+    if all_cores:
+        nproc = os.cpu_count() or 1
+        workers = max(1, min(nproc, one.n_q_heads))
+        _ORACLE_STATE.update(O=O, T=T)
+        tp = []
+        with mp.get_context("fork").Pool(workers) as pool:
+            for i, qn in enumerate(qs):
+                t0 = time.perf_counter()
+                R = O.route(qn, T.W, T.route_K, T.seg.span_len, one.n_kv_heads, one.top_k)
+                got = pool.map(_oracle_head, [(h, qn, R.ids) for h in range(one.n_q_heads)], chunksize=1)
+                dt = time.perf_counter() - t0
+                if i >= warmup:
+                    tp.append(dt)
+                if i == len(qs) - 1:
+                    par = np.stack([g[1] for g in sorted(got, key=lambda g: g[0])])
+                    assert np.array_equal(par, ref), "the forked oracle must reproduce the single-thread result"
+        res.update(sec_all=float(np.mean(tp)), cores_all=workers, nproc=nproc)
     del limiter
-    sec = float(np.mean(times))
-    desc = (f"1 of {spec.batch} sequences x 1 of {spec.n_layers} layers of configs[{spec.config_id}] "
-            f"({spec.contexts[0]} tokens, m={T.seg.m} spans, A={T.seg.A} pool tokens, all {spec.n_q_heads} q heads): "
-            f"oracle route + mixed attention per step, numpy fp64, 1 thread; scaled x{spec.batch} sequences")
-    return sec, desc
+    res["desc"] = (f"1 of {spec.batch} sequences x 1 of {spec.n_layers} layers of configs[{spec.config_id}] "
+                   f"({spec.contexts[0]} tokens, m={T.seg.m} spans, A={T.seg.A} pool tokens, all {spec.n_q_heads} q heads): "
+                   f"oracle route + mixed attention per step, numpy fp64; scaled x{spec.batch} sequences")
+    return res
+
+
+def oracle_sample_subprocess(config: int, steps: int, warmup: int, rho: float):
+    """The all-cores leg forks a process pool: it runs in a fresh interpreter that never touched CUDA."""
+    import subprocess
+    arg = json.dumps({"config": config, "steps": steps, "warmup": warmup, "rho": rho})
+    r = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-worker", arg], capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("oracle worker failed: " + r.stderr[-2000:])
+    return json.loads(r.stdout.strip().splitlines()[-1])
 
 
 def run_reference(args):
@@ -134,11 +203,14 @@ def run_reference(args):
     if rank != 0:
         return
     spec = get_spec(args.config)
-    sec, desc = oracle_sample(spec, args.steps, args.warmup, args.rho)
+    res = oracle_sample(spec, args.steps, args.warmup, args.rho)
+    sec, desc = res["sec_1"], res["desc"] + "; 1 thread"
     us_layer_step = sec * spec.batch * 1e6
     line = {
         "impl": "reference", "metric": METRIC, "value": us_layer_step, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": us_layer_step * spec.n_layers / 1e3,
+        "steps": args.steps, "warmup": args.warmup,
+        # extrapolated like `value`: the arm times 1 sequence x 1 layer per step (see cpu_baseline.sample)
+        "ms_per_step": us_layer_step * spec.n_layers / 1e3, "ms_per_step_is": "extrapolated from the sample",
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": spec.name, "batch": spec.batch, "context": spec.contexts[0], "layers": spec.n_layers,
                    "rank": spec.rank, "top_k": spec.top_k, "rho": args.rho},
@@ -223,18 +295,25 @@ def run_ours(args):
     torch.cuda.empty_cache()
     t_setup = time.time() - t_setup
 
+    fused, why = eng.sekv_get_path()
+    if not args.generic and not fused:
+        raise SystemExit("bench.py: the batch does not run on the fused layer kernel: " + why)
+
     L, Bn, Hq = spec.n_layers, spec.batch, spec.n_q_heads
-    n_q = args.warmup + args.steps + args.profile_steps + args.e2e_steps + 4
-    q_all = [make_queries(spec, 0, dev)]
-    for i in range(1, n_q):
-        q_all.append(next_queries_ar1(spec, q_all[-1], i, args.rho))
-    q_cur = torch.empty_like(q_all[0])
     out = torch.empty((L, Bn, Hq, 128), dtype=eng.out_dtype, device=dev)
     static_bytes = eng.sekv_static_bytes_per_layer()
     esz = eng.esize
+    q_cur = torch.empty((L, Bn, Hq, 128), dtype=eng.st_dtype, device=dev)
+    stream_state = {"q": make_queries(spec, 0, dev), "i": 0}
 
-    def step(i):
-        q_cur.copy_(q_all[i])
+    def next_q(rho):
+        """next query of the AR(1) stream (device-side synthesis, outside every timed region)"""
+        stream_state["i"] += 1
+        stream_state["q"] = next_queries_ar1(spec, stream_state["q"], stream_state["i"], rho)
+        return stream_state["q"]
+
+    def step(q):
+        q_cur.copy_(q)
         eng.sekv_decode_step(q_cur, spec.top_k, out)
 
     def barrier():
@@ -242,81 +321,53 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def timed(rho, n_warm, n_steps):
+        """n_warm untimed steps of the rho stream (the cache reaches its steady state), then n_steps timed ones:
+        device time (CUDA events on the launching stream), statistics of the timed steps only."""
+        for _ in range(n_warm):
+            step(next_q(rho))
+        qs = [next_q(rho) for _ in range(n_steps)]
+        barrier()
+        eng.sekv_reset_stats()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for q in qs:
+            step(q)
+        e1.record()
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1), world, dev), eng.sekv_get_stats()
+
+    def algo_bytes_of(st, n_layer_steps):
+        return n_layer_steps * static_bytes - st["coarse_rows_skipped"] * 2 * 128 * esz + st["factor_bytes_algo"]
+
+    # ---- pinned host -> device bandwidth (what the factor fetch is measured against) -----------------
+    pin = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+    dst = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    best = 0.0
+    for _ in range(5):
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(); dst.copy_(pin, non_blocking=True); a1.record(); torch.cuda.synchronize()
+        best = max(best, (256 << 20) / (a0.elapsed_time(a1) * 1e-3) / 1e9)
+    pcie_h2d_gbs = best
+    del pin, dst
+
     # ---- device-resident timing (value) ---------------------------------------------------------
-    qi = 0
-    for _ in range(max(args.warmup, 3)):
-        step(qi); qi += 1
-    barrier()
-    eng.sekv_reset_stats()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.01)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        step(qi); qi += 1
-    e1.record()
-    barrier()
+    ms, st = timed(args.rho, max(args.warmup, 3), args.steps)
     sampler.stop_flag = True
-    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
     sampler.join(timeout=2)
-    st = eng.sekv_get_stats()
     layer_steps = args.steps * L
     us_layer_step = replica_us_per_layer_step(ms, args.steps, L, world)   # aggregate over replicas
-    algo_bytes = layer_steps * static_bytes - st["coarse_rows_skipped"] * 2 * 128 * esz + st["factor_bytes_algo"]
+    algo_bytes = algo_bytes_of(st, layer_steps)
     hbm_gbs = algo_bytes / (ms * 1e-3) / 1e9 * world
     hit = st["cache_hits"] / max(1, st["zoomed_spans"])
     launches = st["kernel_launches"] + args.steps            # + the q staging copy per step
 
-    # ---- per-kernel profile (CUDA events around every kernel, eager launches) ----------------------
-    eng.sekv_set_profiling(True)
-    step(qi); qi += 1                                        # warm the eager path
-    eng.sekv_get_kernel_times()
-    eng.sekv_reset_stats()
-    for _ in range(args.profile_steps):
-        step(qi); qi += 1
-    kt = eng.sekv_get_kernel_times()
-    st_p = eng.sekv_get_stats()
-    eng.sekv_set_profiling(False)
-    tot_kernel_ms = sum(v["ms"] for k, v in kt.items() if k not in ("fetch", "prefetch"))
-    peak, peak_src = measured_peaks()
-    prof_layer_steps = max(1, st_p["layer_steps"])
-    if kt["fused"]["launches"]:
-        # ONE kernel per layer-step does a1-a7: its algorithmic bytes are the layer-step's (SURVEY.md 8(d))
-        dom, dom_name = kt["fused"], "fused_layer_kernel (a1-a7: route, plan, pool/coarse/zoom partials, combine)"
-        dom_bytes = (prof_layer_steps * static_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz
-                     + st_p["factor_bytes_algo"]) / prof_layer_steps
-    else:
-        dom, dom_name = kt["stage1"], "stage1 kernel (a5: pool + coarse entries)"
-        rows_bytes = sum(2 * spec.n_kv_heads * (a + m) * 128 * esz for a, m in zip(eng.pool_per_seq, eng.spans_per_seq))
-        dom_bytes = rows_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz / prof_layer_steps + Bn * Hq * 128 * esz
-    eager_us = max(dom["ms"] * 1e3 / max(1, dom["launches"]), 1e-9)
-    fused = bool(kt["fused"]["launches"])
-    if fused and world == 1:
-        # the layer kernel is the only kernel on the launching stream inside the timed region (the prefetch
-        # kernels run on the side stream): its average launch duration over the timed region, CUDA events on
-        # that stream, is the step time / 32 -- launch gaps between the dependent kernels included
-        dom_us = ms * 1e3 / layer_steps
-        dom_bytes = algo_bytes / layer_steps
-        timing = "CUDA events on the launching stream over the timed region (%d steps x %d launches, one graph per step)" % (args.steps, L)
-    else:
-        dom_us = eager_us
-        timing = "CUDA events on the launching stream around every launch, eager launches, %d steps" % args.profile_steps
-    roofline = {"bound": "hbm", "kernel": dom_name,
-                "achieved": dom_bytes / (dom_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
-                "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak,
-                # dram__bytes_read.sum + dram__bytes_write.sum per launch of the layer kernel, from the one
-                # `ncu --set full` capture summarised in profiles/r01_fused_layer_kernel_ncu_full.md
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH if fused and not args.layers and args.config == 2 else None,
-                "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_us": dom_us,
-                "share_of_step_kernel_time": dom["ms"] / max(1e-9, tot_kernel_ms),
-                "timing": timing,
-                "kernel_us_per_launch_eager": {k: v["ms"] * 1e3 / v["launches"] for k, v in kt.items() if v["launches"]}}
-
-    # ---- end to end through host buffers -----------------------------------------------------------------
-    q_host = [q_all[qi + i].cpu().pin_memory() for i in range(args.e2e_steps)]
+    # ---- end to end through host buffers, same stream, same stationary state --------------------------
+    q_host = [next_q(args.rho).cpu().pin_memory() for _ in range(args.e2e_steps)]
     out_host = torch.empty(out.shape, dtype=out.dtype).pin_memory()
     eng.sekv_decode_step_host(q_host[0], spec.top_k, out_host)
     eng.sekv_reset_stats()
@@ -325,20 +376,87 @@ def run_ours(args):
     for i in range(args.e2e_steps):
         eng.sekv_decode_step_host(q_host[i], spec.top_k, out_host)
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = max_over_ranks(e2e_s, world, dev)
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
     st_e = eng.sekv_get_stats()
+    fetch_e = (st_e["h2d_bytes"] + st_e["prefetch_h2d_bytes"]) // max(1, args.e2e_steps)
     e2e = {"value": e2e_s * 1e6 / (args.e2e_steps * L) / world, "unit": UNIT,
-           "h2d_bytes_per_step": q_host[0].numel() * esz + st_e["h2d_bytes"] // max(1, args.e2e_steps),
+           "h2d_bytes_per_step": q_host[0].numel() * esz + fetch_e,
            "d2h_bytes_per_step": out_host.numel() * out_host.element_size(),
-           "factor_fetch_bytes_per_step": st_e["h2d_bytes"] // max(1, args.e2e_steps), "steps": args.e2e_steps}
+           "factor_fetch_bytes_per_step": fetch_e, "steps": args.e2e_steps}
+
+    # ---- rho sweep: the miss volume at which the fetch stays hidden ------------------
+    sweep = []
+    if args.sweep_steps > 0 and world == 1:
+        for rho in (1.0, 0.99, 0.9, 0.0):
+            ms_r, st_r = timed(rho, 10, args.sweep_steps)
+            us_r = ms_r * 1e3 / (args.sweep_steps * L)
+            sweep.append({"rho": rho, "value": us_r, "steps": args.sweep_steps,
+                          "hit_rate": st_r["cache_hits"] / max(1, st_r["zoomed_spans"]),
+                          "demand_h2d_mb_per_step": st_r["h2d_bytes"] / args.sweep_steps / 1e6,
+                          "prefetch_h2d_mb_per_step": st_r["prefetch_h2d_bytes"] / args.sweep_steps / 1e6,
+                          "pcie_ms_per_step_at_measured_bw": (st_r["h2d_bytes"] + st_r["prefetch_h2d_bytes"]) / args.sweep_steps
+                                                             / (pcie_h2d_gbs * 1e9) * 1e3,
+                          "ms_per_step": ms_r / args.sweep_steps})
+        for e in sweep:
+            e["fetch_exposed_us"] = e["value"] - sweep[0]["value"]       # against 100% hits
+    value_all_hits = sweep[0]["value"] if sweep else None
+
+    # ---- per-kernel profile (CUDA events around every kernel, eager launches) ----------------------
+    eng.sekv_set_profiling(True)
+    step(next_q(args.rho))                                   # warm the eager path
+    eng.sekv_get_kernel_times()
+    eng.sekv_reset_stats()
+    for _ in range(args.profile_steps):
+        step(next_q(args.rho))
+    kt = eng.sekv_get_kernel_times()
+    st_p = eng.sekv_get_stats()
+    eng.sekv_set_profiling(False)
+    tot_kernel_ms = sum(v["ms"] for k, v in kt.items() if k not in ("fetch", "prefetch"))
+    peak, peak_src = measured_peaks()
+    prof_layer_steps = max(1, st_p["layer_steps"])
+    is_fused = bool(kt["fused"]["launches"])
+    if is_fused:
+        # ONE kernel per layer-step does a1-a7: its algorithmic bytes are the layer-step's (SURVEY.md 8(d))
+        dom, dom_name = kt["fused"], "fused_layer_kernel (a1-a7: route, plan, pool/coarse/zoom partials, combine)"
+        dom_bytes = algo_bytes_of(st_p, prof_layer_steps) / prof_layer_steps
+    else:
+        dom, dom_name = kt["stage1"], "stage1 kernel (a5: pool + coarse entries)"
+        rows_bytes = sum(2 * spec.n_kv_heads * (a + m) * 128 * esz for a, m in zip(eng.pool_per_seq, eng.spans_per_seq))
+        dom_bytes = rows_bytes - st_p["coarse_rows_skipped"] * 2 * 128 * esz / prof_layer_steps + Bn * Hq * 128 * esz
+    eager_us = max(dom["ms"] * 1e3 / max(1, dom["launches"]), 1e-9)
+    if is_fused and world == 1:
+        # the layer kernel is the only kernel on the launching stream inside the timed region: its average launch
+        # duration over the timed region, CUDA events on that stream, is the step time / layers -- the gaps
+        # between the dependent kernels included
+        dom_us = ms * 1e3 / layer_steps
+        dom_bytes = algo_bytes / layer_steps
+        timing = "CUDA events on the launching stream over the timed region (%d steps x %d launches, one graph per step)" % (args.steps, L)
+    else:
+        dom_us = eager_us
+        timing = "CUDA events on the launching stream around every launch, eager launches, %d steps" % args.profile_steps
+    traffic, traffic_src = (None, "not quoted for this configuration")
+    if is_fused and not args.layers and args.config == 2:
+        traffic, traffic_src = ncu_traffic_per_launch()
+    roofline = {"bound": "hbm", "kernel": dom_name,
+                "achieved": dom_bytes / (dom_us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": dom_bytes / (dom_us * 1e-6) / 1e9 / peak,
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch of the layer kernel from the tracked
+                # `ncu --set full` capture (null when the kernel has changed since)
+                "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_us": dom_us,
+                "share_of_step_kernel_time": dom["ms"] / max(1e-9, tot_kernel_ms),
+                "timing": timing,
+                "kernel_us_per_launch_eager": {k: v["ms"] * 1e3 / v["launches"] for k, v in kt.items() if v["launches"]}}
 
     if rank != 0:
         return
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        sec, desc = oracle_sample(spec, 3, 1, args.rho)
-        cpu_baseline = {"value": sec * spec.batch * 1e6, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
+        r = oracle_sample_subprocess(args.config, 2, 1, args.rho)
+        cpu_baseline = {"value": r["sec_all"] * spec.batch * 1e6, "unit": UNIT, "cores": r["cores_all"], "kind": "oracle",
+                        "sample": r["desc"] + "; one forked process per query head over the host cores",
+                        "nproc": r.get("nproc"), "value_1_thread": r["sec_1"] * spec.batch * 1e6}
     n_ctas, parts = eng.sekv_get_schedule()
     line = {
         "metric": METRIC, "value": us_layer_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -350,14 +468,21 @@ def run_ours(args):
                    "kv_heads": spec.n_kv_heads, "rank": spec.rank, "top_k": spec.top_k, "rho": args.rho,
                    "spans_per_seq": eng.spans_per_seq, "pool_per_seq": eng.pool_per_seq,
                    "cache_ways": cfg.cache_ways, "cache_hit_rate": hit, "graph": not args.no_graph,
-                   "kernels": "generic multi-kernel" if args.generic else "one persistent kernel per layer-step: warp workers on two dependency-ordered queues (mma.sync bf16, cp.async K/V ring, TMA bulk factor copies)",
+                   "path": "fused layer kernel" if fused else "generic multi-kernel path (" + why + ")",
+                   "kernels": "generic multi-kernel" if args.generic else "one persistent kernel per layer-step: a team of warps runs route / top-k / cache plan in shared memory, warp workers claim POOL / COARSE / ZOOM / COMBINE items (mma.sync bf16, cp.async K/V ring, TMA bulk copies of factor chunks and routing rows)",
                    "prefetch": cfg.prefetch, "stage1_ctas": n_ctas,
                    "l2": "inputs larger than L2: one step streams %.2f GB of tables (L2 = 126 MB), no flush" % (algo_bytes / args.steps / 1e9),
                    "replicas": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
                    "setup_s": round(t_setup, 1)},
         "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-        "fetch": {"h2d_bytes_per_step": st["h2d_bytes"] / args.steps, "misses_per_step": st["cache_misses"] / args.steps,
-                  "zoomed_per_step": st["zoomed_spans"] / args.steps},
+        "fetch": {"pcie_h2d_gbs": pcie_h2d_gbs,
+                  "demand_h2d_bytes_per_step": st["h2d_bytes"] / args.steps,
+                  "prefetch_h2d_bytes_per_step": st["prefetch_h2d_bytes"] / args.steps,
+                  "misses_per_step": st["cache_misses"] / args.steps, "zoomed_per_step": st["zoomed_spans"] / args.steps,
+                  "value_at_100pct_hits": value_all_hits,
+                  "fetch_exposed_us": (us_layer_step - value_all_hits) if value_all_hits is not None else None,
+                  "overlap": "demand misses are read by the bulk-copy engine inside the layer kernel; the speculative prefetch of layer l is copied inside layer l+1's kernel"},
+        "sweep": sweep,
     }
     if cpu_baseline:
         line["cpu_baseline"] = cpu_baseline
@@ -368,6 +493,11 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse()
+    if a.oracle_worker:
+        from workloads import get_spec as _gs
+        w = json.loads(a.oracle_worker)
+        print(json.dumps(oracle_sample(_gs(w["config"]), w["steps"], w["warmup"], w["rho"], all_cores=True)))
+        sys.exit(0)
     if a.impl == "reference":
         run_reference(a)
     else:
