@@ -470,9 +470,10 @@ __device__ __forceinline__ void publish_mask(const FusedParams& P, const Team& T
 // this layer's kernel.  Also: zoom bit-mask for the COARSE items (an expanded span's coarse entry is
 // replaced by its tokens), de-duplication of caller-supplied ids, one descriptor per
 // expanded span for the ZOOM items, statistics.
-__device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
+__device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T_in, const PlanTables& t, int bg, int span0,
                                           int m, int n_zoom, int n_cand, bool dedupe, uint32_t epoch,
-                                          bool mask_done, unsigned long long* tm = nullptr) {
+                                          bool mask_done, bool solo_tail, unsigned long long* tm = nullptr) {
+  Team T = T_in;
   const int g = bg % P.Hkv, ways = P.ways;
   int32_t* tags = P.lv.tags + (size_t)bg * ways;
   uint32_t* stamps = P.lv.stamps + (size_t)bg * ways;
@@ -529,6 +530,31 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   n_need = min(n_need, ways);
   if (!mask_done) publish_mask(P, T, t, bg, epoch);
   if (T.tt == 0) { P.plan_counts[2 * bg] = n_zoom; P.plan_counts[2 * bg + 1] = n_cand; }
+  // statistics of pass 1 (every warp its own share)
+  n_hit = warp_sum_i(n_hit); n_miss = warp_sum_i(n_miss);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
+    bytes_demand += __shfl_xor_sync(0xffffffffu, bytes_demand, o);
+  }
+  if (T.lane == 0) {
+    if (n_hit) atomicAdd(&P.stats[ST_HITS], (unsigned long long)n_hit);
+    if (n_miss) atomicAdd(&P.stats[ST_MISSES], (unsigned long long)n_miss);
+    if (n_hit + n_miss) {
+      atomicAdd(&P.stats[ST_ZOOMED], (unsigned long long)(n_hit + n_miss));
+      atomicAdd(&P.stats[ST_SKIPPED], (unsigned long long)(n_hit + n_miss));
+    }
+    if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
+    if (bytes_demand) atomicAdd(&P.stats[ST_H2D], bytes_demand);
+  }
+  // The mask and the descriptors of the hits are out: what is left (slots for the misses, the cache tables) is
+  // little and serial.  With solo_tail the team's warps 1.. leave here for the work queue and warp 0 finishes
+  // alone (the tables sit in its own region).
+  if (solo_tail) {
+    team_bar(T);
+    if (T.tw != 0) return;
+    T.tt = T.lane; T.ts = 32; T.ntw = 1;
+  }
   // victims: the n_need oldest ways not used by this step (ties to the lower way), by repeated extraction
   // of the minimum (stamp, way) -- only as many as this step has misses
   if (T.tw == 0) {
@@ -575,23 +601,11 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T, c
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
-  // statistics (off the critical path)
-  n_hit = warp_sum_i(n_hit); n_miss = warp_sum_i(n_miss); n_pf_slot = warp_sum_i(n_pf_slot);
+  // statistics of pass 2
+  n_pf_slot = warp_sum_i(n_pf_slot);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    bytes_algo += __shfl_xor_sync(0xffffffffu, bytes_algo, o);
-    bytes_demand += __shfl_xor_sync(0xffffffffu, bytes_demand, o);
-    bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
-  }
+  for (int o = 16; o > 0; o >>= 1) bytes_pf += __shfl_xor_sync(0xffffffffu, bytes_pf, o);
   if (T.lane == 0) {
-    if (n_hit) atomicAdd(&P.stats[ST_HITS], (unsigned long long)n_hit);
-    if (n_miss) atomicAdd(&P.stats[ST_MISSES], (unsigned long long)n_miss);
-    if (n_hit + n_miss) {
-      atomicAdd(&P.stats[ST_ZOOMED], (unsigned long long)(n_hit + n_miss));
-      atomicAdd(&P.stats[ST_SKIPPED], (unsigned long long)(n_hit + n_miss));
-    }
-    if (bytes_algo) atomicAdd(&P.stats[ST_FACTOR_ALGO], bytes_algo);
-    if (bytes_demand) atomicAdd(&P.stats[ST_H2D], bytes_demand);
     if (bytes_pf) atomicAdd(&P.stats[ST_PF_BYTES], bytes_pf);
     if (n_pf_slot) atomicAdd(&P.stats[ST_PREFETCHED], (unsigned long long)n_pf_slot);
   }
@@ -692,7 +706,7 @@ __device__ __forceinline__ void select_team(const FusedParams& P, const Team& T,
 // ---------------------------------------------------------------------------------------------------
 template <int G>
 __device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int bg, uint32_t& epoch, bool pdl_wait,
-                                            unsigned long long* tm) {
+                                            bool solo_tail, unsigned long long* tm) {
   const PlanTables t = plan_tables(P, T.tab);
   uint32_t* keys = reinterpret_cast<uint32_t*>(T.tab + P.sm_keys);
   float* sqp = reinterpret_cast<float*>(T.tab + P.sm_qp);
@@ -711,7 +725,7 @@ __device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int b
       team_bar(T);
       publish_mask(P, T, t, bg, epoch);
       mark(tm, 3, T.tt);
-      plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch, true, tm);
+      plan_team(P, T, t, bg, span0, m, cnt, n_cand, false, epoch, true, solo_tail, tm);
     }
   } else {
     // caller-supplied zoom set (sekv_decode_attn)
@@ -726,7 +740,7 @@ __device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int b
     team_bar(T);
     plan_init_scatter(P, T, t, m);
     team_bar(T);
-    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch, false);
+    plan_team(P, T, t, bg, span0, m, cnt, cnt, true, epoch, false, solo_tail);
   }
 }
 
@@ -1437,8 +1451,12 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
     for (int bg = (int)blockIdx.x; bg < P.BG; bg += (int)gridDim.x) {
       unsigned long long t0 = 0ull;
       if (P.trace) { t0 = globaltimer_ns(); if (lane == 0) { tm[0] = t0; tm[1] = t0; tm[2] = t0; tm[3] = t0; } }
-      chain_group<G>(P, T, bg, epoch, pdl_wait, tm);
+      // the last group of this CTA: once its mask and hit descriptors are out, warps 1.. go on to the work queue
+      // (only when the team's tables fit warp 0's own region: the released warps reuse theirs)
+      const bool solo_tail = (P.mode & FM_ATTN) && bg + (int)gridDim.x >= P.BG && P.sm_stage <= P.region_bytes;
+      chain_group<G>(P, T, bg, epoch, pdl_wait, solo_tail, tm);
       pdl_wait = false;
+      if (solo_tail && warp != 0) break;
       const int rec = P.main_end + bg;                         // trace record after the queue items
       if (P.trace && tid == 0 && rec < P.trace_cap) {
         unsigned long long* r = P.trace + 8 * (size_t)rec;
@@ -1447,7 +1465,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
         r[2] = t0; r[3] = globaltimer_ns();
         r[4] = tm[0]; r[5] = tm[1]; r[6] = tm[2]; r[7] = tm[3];
       }
-      team_bar(T);                                             // the tables are free for the next group
+      if (!solo_tail) team_bar(T);                             // the tables are free for the next group
     }
     phase = T.ph[0]; phase1 = T.ph[1];                         // the items go on with this warp's barriers
   }
