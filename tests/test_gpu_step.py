@@ -145,3 +145,55 @@ def test_item_trace_records_every_work_item():
     assert eng.sekv_set_trace(None) == n
     assert torch.equal(out0, out1)
     eng.close()
+
+
+def test_soak_200_steps_graph_replay_misses_evictions_prefetch():
+    """200 graph-replayed steps of configs[2] at its full per-layer size (two layers built) at rho = 0.9: ~12% demand
+    misses per step, evictions, write-backs and prefetch copies carried by the next layer's kernel.  Every step: the
+    cache statistics add up and the outputs are finite; the LAST step, reached through all that cache traffic, is
+    compared with the oracle (every zoom set, sampled heads).  (compute-sanitizer is closed on the GPU pool: this
+    is the long-run check of the kernel's polls, stamps and cross-proxy hand-offs.)"""
+    from paper_2606_31145_b200 import engine as E
+    from paper_2606_31145_b200.export import export_tables
+    spec = get_spec(2).with_(n_layers=2)
+    lay = make_layouts(spec)
+    eng = E.create_engine(spec, lay, gen_device="cuda", prefetch=8, use_graph=1, out_dtype="bf16")
+    assert eng.sekv_get_path()[0]
+    L, B, Hq, Hkv = spec.n_layers, spec.batch, spec.n_q_heads, spec.n_kv_heads
+    q = make_queries(spec, 0, "cuda")
+    q_cur = torch.empty_like(q)
+    out = torch.zeros((L, B, Hq, 128), dtype=eng.out_dtype, device="cuda")
+    n_steps = 200
+    for step in range(n_steps):
+        q_cur.copy_(q)
+        eng.sekv_decode_step(q_cur, spec.top_k, out)
+        if step % 20 == 19 or step == n_steps - 1:
+            torch.cuda.synchronize()
+            assert torch.isfinite(out.float()).all(), step
+            st = eng.sekv_get_stats()
+            assert st["layer_steps"] == (step + 1) * L
+            assert st["zoomed_spans"] == (step + 1) * L * B * Hkv * spec.top_k == st["cache_hits"] + st["cache_misses"]
+        if step < n_steps - 1:
+            q = next_queries_ar1(spec, q, step + 1, 0.9)
+    assert eng.sekv_graph_count() == 1
+    st = eng.sekv_get_stats()
+    assert st["cache_misses"] > 200 * 50 and st["prefetched_spans"] > 0 and st["cache_hits"] > st["cache_misses"]
+    qn = to_np(q)
+    out_h = out.float().cpu().numpy().astype(np.float64)
+    hs = [0, 5, 18, 31]
+    for l in range(L):
+        ids, count = eng.sekv_last_zoom_ids(l)
+        torch.cuda.synchronize()
+        ids_h, count_h = ids.cpu().numpy(), count.cpu().numpy()
+        for b in (0, 3):
+            T = tables_from_export(export_tables(eng, l, b), Hq, Hkv, spec.route_dim)
+            R = O.route(qn[l, b], T.W, T.route_K, T.seg.span_len, Hkv, spec.top_k)
+            zoom = []
+            for g in range(Hkv):
+                c = int(count_h[b, g])
+                check_ids(ids_h[b, g, :c], R.ids[g], R.group_logit[g])
+                zoom.append([int(x) for x in ids_h[b, g, :c]])
+            ref, _ = O.decode_attn(qn[l, b], T, zoom, heads=hs)
+            assert rel_l2(out_h[l, b, hs], ref[hs]) <= TOL_BF16["rel_l2"], (l, b)
+            assert np.abs(out_h[l, b, hs] - ref[hs]).max() <= TOL_BF16["max_abs"]
+    eng.close()
