@@ -552,7 +552,21 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T_in
   // alone (the tables sit in its own region).
   if (solo_tail) {
     team_bar(T);
-    if (T.tw != 0) return;
+    if (T.tw != 0) {
+      // On the way out: pull the resident blobs of the zoom set towards L2 (one prefetch per 128-byte line, fire and
+      // forget).  The ZOOM items run a few microseconds from now, after the COARSE items, and HBM is idle meanwhile.
+      for (int j = T.tw - 1; j < n_zoom; j += T.ntw - 1) {
+        const int id = t.sh_ids[j];
+        if (id < 0) continue;
+        const int way = t.way_of[id];
+        if (way < 0) continue;
+        const uint32_t meta = t.meta[id];
+        const uint32_t lines = (uint32_t)(blob_dims(2, (int)(meta >> 16), meta & 0xff, (meta >> 8) & 0xff).bytes >> 7);
+        const uint8_t* base = P.lv.slots + ((size_t)bg * ways + way) * P.slot_bytes;
+        for (uint32_t i = T.lane; i < lines; i += 32) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + ((size_t)i << 7)));
+      }
+      return;
+    }
     T.tt = T.lane; T.ts = 32; T.ntw = 1;
   }
   // victims: the n_need oldest ways not used by this step (ties to the lower way), by repeated extraction
@@ -713,7 +727,6 @@ __device__ __forceinline__ void chain_group(const FusedParams& P, Team& T, int b
   int span0, m;
   if (P.mode & FM_ROUTE) {
     route_team<G>(P, T, bg, keys, sqp, t, &span0, &m, pdl_wait, tm);
-    if (pdl_wait) epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
     int cnt, n_cand;
     select_team(P, T, t, keys, m, &cnt, &n_cand, tm);
     int32_t* my_ids = P.ids + (size_t)bg * max(P.k_cap, 1);
@@ -1434,14 +1447,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
       if (first.kind == IT_POOL) { rows_prefill(P, first, region, lane); prefilled = true; }
     }
   }
-  if (!is_team || !P.hoist) {
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
-  }
-  // The layer's launch sequence number picks the counter set.  (It is only written by launches of this layer: a
-  // hoisted team, which has not waited yet, follows another layer's kernel and reads a settled value.)
+  // The layer's step stamp and launch sequence number (which picks the counter set) are only written by launches
+  // of THIS layer.  With P.hoist the kernel before this one on the stream is the previous layer's of the same
+  // step, so both are settled and can be read before the wait; otherwise after it.
+  if (!P.hoist) asm volatile("griddepcontrol.wait;" ::: "memory");
+  epoch = *reinterpret_cast<volatile const uint32_t*>(P.lv.layer_step) + 1u;
   const uint32_t seq = *reinterpret_cast<volatile const uint32_t*>(P.ctrs);
   int32_t* ctrs = P.ctrs + 4 + (seq & 1u) * P.ctrs_set;
+  if (P.hoist && !is_team) asm volatile("griddepcontrol.wait;" ::: "memory");
   if (is_team) {
     Team T;
     T.tt = tid; T.ts = ntw * 32; T.lane = lane; T.tw = warp; T.ntw = ntw; T.scratch = team_scratch;
@@ -1736,9 +1749,10 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.zmask2 = (uint2*)ws(h, h->F.off_zmask2) + (size_t)layer * c.max_seqs * c.n_kv_heads * h->mask_words;
   // the chain (a1-a4) runs whenever there is routing to do or a zoom set to plan
   P.has_chain = ((mode & FM_ROUTE) || c.k_cap > 0) ? 1 : 0;
-  // whole-step launches of a model with more than one layer: the previous kernel on the stream is another layer's
-  // (it writes none of this layer's tables), so the chain's static part may run before the dependency wait
-  P.hoist = ((mode & FM_ROUTE) && (mode & FM_ATTN) && c.n_layers > 1) ? 1 : 0;
+  // layers 1.. of a whole-step launch: the kernel before this one on the stream is the previous layer's of the same
+  // step (it writes none of this layer's tables), so the chain's static part, the step stamp and the sequence
+  // number may be read before the dependency wait.  Layer 0 follows whatever the caller ran last: no hoisting.
+  P.hoist = ((mode & FM_ROUTE) && (mode & FM_ATTN) && layer > 0) ? 1 : 0;
   if ((mode & FM_ROUTE) && (mode & FM_ATTN)) {                  // whole-step launches run the layers in order
     const LayerView nv = layer_view(h, (layer + 1) % c.n_layers);
     P.next_W = (const uint8_t*)nv.W;
