@@ -4,7 +4,7 @@
 //   chain (a1-a4), per (sequence, kv head) group bg, by a TEAM of warps of CTA bg % grid, entirely in
 //   shared memory (no global round trips between the steps):
 //     q' = W q (Eq. 4, tensor cores)  ->  x = q'.K_bar/sqrt(d') + ln|S|, X = max over the group (Eq. 5, GQA;
-//     the routing table streams through a cp.async double buffer)  ->  top-k by radix select (Eq. 9, cap
+//     the routing table streams through bulk-copied staging buffers)  ->  top-k by radix select (Eq. 9, cap
 //     L123; ties to the lower span id)  ->  residency plan of the device factor cache (LRU), zoom bit-mask,
 //     one stamped descriptor per expanded span
 //   work items (a5-a7), one warp each, claimed in queue order:
@@ -12,8 +12,10 @@
 //     COARSE  (b, g, rows)   partial over the coarse entries (+ln|S|) of the spans that are NOT expanded
 //                            (an expanded span's coarse entry is replaced by its tokens); waits
 //                            for the group's zoom mask
-//     ZOOM    (b, g, spans)  expanded spans through the factored form (Eq. 8 never materialised); waits for
-//                            the span's descriptor; the U factors move by 1-D bulk copies (TMA engine)
+//     ZOOM    (b, g, 1 span) an expanded span through the factored form (Eq. 8 never materialised); waits for
+//                            the span's descriptor; the U factors move by 1-D bulk copies (TMA engine); a demand
+//                            miss reads its blob from the pinned-host store over PCIe and keeps it in its slot
+//     PREFETCH (b, g, i)     speculative: a candidate of the PREVIOUS layer's plan, pinned host -> cache slot
 //     COMBINE (b, h)         log-sum-exp merge of the head's partials -> output (L61)
 //
 // Waiting items only wait on the teams (which start at t = 0 and wait on nobody) or on items earlier in the
@@ -126,32 +128,10 @@ __device__ __forceinline__ void wait_field(const int32_t* c, int shift, int targ
   __syncwarp();
 }
 
-// spin (lane 0) until the counter reaches `target`
-// (relaxed polls -- an acquire load would flush L1 on every poll -- then one acquire fence)
-__device__ __forceinline__ void wait_ctr(const int32_t* c, int target, int lane, unsigned long long* t_mid = nullptr) {
-  if (lane == 0) {
-    int v;
-    for (;;) {
-      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(c) : "memory");
-      if (v >= target) break;
-      __nanosleep(64);
-    }
-    asm volatile("fence.acq_rel.gpu;" ::: "memory");
-    if (t_mid) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(*t_mid));
-  }
-  __syncwarp();
-}
 // trace mark k (0..3) of the current item (lane 0; tm = null when tracing is off)
 __device__ __forceinline__ void mark(unsigned long long* tm, int k, int lane) {
   if (tm && lane == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tm[k]));
 }
-// every lane's earlier global writes happen-before the counter increment: __syncwarp orders them before
-// lane 0's release (cumulativity), so no separate fence is needed
-__device__ __forceinline__ void signal_ctr(int32_t* c, int lane) {
-  __syncwarp();
-  if (lane == 0) red_add_release(c, 1);
-}
-
 // Q fragments of the group's heads (rows gid < G; zero rows above): qf[j] = q[gid][8 (t4 + 4 j) .. +7]
 __device__ __forceinline__ void load_q_frags(const __nv_bfloat16* __restrict__ q, int G, int gid, int t4,
                                              uint32_t (&qf)[4][4]) {
@@ -269,7 +249,6 @@ __device__ __forceinline__ PlanTables plan_tables(const FusedParams& P, uint8_t*
 // Tables that need nothing from this step's routing -> shared memory by 4-byte cp.async copies, all in flight at
 // once (no register round trip): span meta (the directory word carries |S| and both ranks), ln|S|, cache tags and
 // stamps.  The caller commits / waits and runs a team barrier; _scatter then inverts the tags into way_of.
-__device__ __forceinline__ void r_select_end(unsigned long long*) {}
 __device__ __forceinline__ void plan_init_fill(const FusedParams& P, const Team& T, const PlanTables& t, int bg, int span0,
                                                int m) {
   const int g = bg % P.Hkv;
@@ -976,8 +955,6 @@ __device__ __forceinline__ void rows_item(const FusedParams& P, const Item& I, u
   __syncwarp();
   if (lane == 0) red_add_release(grp_ctr(ctrs, bg), kEarlyOne);
 }
-
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 // lane 0 starts a 1-D bulk copy into the warp's region (completion on `bar`); callers wait with mbar_wait
 __device__ __forceinline__ void region_fetch_start(uint8_t* region, const void* src, uint32_t bytes, uint64_t* bar, int lane) {
