@@ -496,11 +496,15 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
   const int n_first = n_chain_cta * (fused_warps() - geo.team_warps) + (h->fused_grid - n_chain_cta) * fused_warps();
   // POOL items: by default sized so that ONE round over the warps that do not start on a chain covers every
   // pool row (they stream while the teams run the chains)
+  // (the copies of the previous layer's prefetch candidates take first-round warps too: see the queue order below)
+  const int n_pf = (c.k_cap > 0 && c.prefetch > 0 && c.n_layers > 1) ? BG * c.prefetch : 0;
+  const int n_first_pool = n_first - n_pf > n_first / 2 ? n_first - n_pf : n_first;
+  const bool pf_first = n_pf > 0 && n_first_pool < n_first;
   int rows = c.item_rows;
   if (rows <= 0) {
     long pool_rows = 0;
     for (int b = 0; b < B; ++b) pool_rows += (long)h->A_b[b] * Hkv;
-    rows = (int)((pool_rows / std::max(n_first, 1) + 1 + 15) / 16 * 16);
+    rows = (int)((pool_rows / std::max(n_first_pool, 1) + 1 + 15) / 16 * 16);
     rows = std::min(256, std::max(32, rows));
   }
   h->fused_item_rows = rows;
@@ -554,14 +558,29 @@ static sekv_status make_fused_schedule(sekv_handle* h) {
         const int kmax = std::min(c.k_cap, h->m_b[b]);
         for (int j0 = 0; j0 < kmax; j0 += zs) attn(zoom_items, IT_ZOOM, b, g, j0, std::min(kmax, j0 + zs));
       }
-  const size_t first = std::min<size_t>((size_t)std::max(n_first, 0), pool_items.size());
-  items.insert(items.end(), pool_items.begin(), pool_items.begin() + first);
+  // Prefetch candidates of the previous layer of the step (copied by this layer's kernel; mostly no-ops).  Their
+  // blobs cross PCIe, and so do the demand misses of THIS layer, which are known only once its chains have run: the
+  // copies go out first (spread over the first round, so that no SM is left without POOL rows to stream) and the
+  // link is free again when the demand misses arrive.
+  std::vector<Item> pf_items;
+  if (n_pf > 0)
+    for (int i = 0; i < c.prefetch; ++i)
+      for (int b = 0; b < B; ++b)
+        for (int g = 0; g < Hkv; ++g) pf_items.push_back(mk(IT_PREFETCH, b, g, i, 0, 0));
+  const size_t first = std::min<size_t>((size_t)std::max(pf_first ? n_first_pool : n_first, 0), pool_items.size());
+  if (pf_first) {
+    const size_t total = first + pf_items.size();
+    size_t ip = 0, ipf = 0;
+    for (size_t i = 0; i < total; ++i) {
+      // slot i takes a copy when the copies are behind their even share
+      if (ipf < pf_items.size() && (ip >= first || ipf * total <= i * pf_items.size())) items.push_back(pf_items[ipf++]);
+      else items.push_back(pool_items[ip++]);
+    }
+  } else {
+    items.insert(items.end(), pool_items.begin(), pool_items.begin() + first);
+    items.insert(items.end(), pf_items.begin(), pf_items.end());
+  }
   h->pool_end = (int)items.size();
-  // prefetch candidates of the previous layer of the step (copied by this layer's kernel; mostly no-ops)
-  if (c.k_cap > 0 && c.prefetch > 0 && c.n_layers > 1)
-    for (int b = 0; b < B; ++b)
-      for (int g = 0; g < Hkv; ++g)
-        for (int i = 0; i < c.prefetch; ++i) items.push_back(mk(IT_PREFETCH, b, g, i, 0, 0));
   // ZOOM positions 0 and 1 of every group first (the plan puts demand misses there: their blobs cross PCIe), then
   // the COARSE items (two tiles each, in flight while the item waits for the zoom mask; ~1 us of work after it),
   // then the other ZOOM items
