@@ -316,6 +316,32 @@ SEKV_API sekv_status sekv_export_span_factors(sekv_handle* h, int32_t layer, int
                                      int32_t* len, int32_t* rank_k, int32_t* rank_v, float* UK, float* sK,
                                      float* VtK, float* UV, float* sV, float* VtV, int32_t* pad_zero);
 
+/* The segmentation counts of sekv_build_sizes (rule of L55, L108, Eq. 17 window) for callers that may not call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  This entry
+ * point allocates NOTHING (no cudaMalloc / cudaFree / allocating library routine, no host allocation): the ~6
+ * bytes per token of scratch that sekv_build_sizes takes from a temporary cudaMalloc live in a file-scope
+ * `static __device__` array of the library, sized for SEKV_STATIC_MAX_TOKENS tokens in SEKV_STATIC_MAX_SEQS
+ * sequences (6.02 MiB; every GPU that loads the library holds it until the process exits).
+ *   cfg: alpha, l_min, window are read (the static fields of sekv_build_sizes; capacities ignored).
+ *   seq_tok_off: HOST int64 [n_seqs+1], seq_tok_off[0] = 0, increasing (copied to the scratch on `stream`).
+ *   H: DEVICE f32 [seq_tok_off[n_seqs]] surprisal.
+ *   counts: DEVICE int32 [n_seqs][2] output = (full-resolution pool tokens A_b, spans m_b) per sequence.
+ *   too_long: DEVICE int32 [1] output = 1 iff some run exceeds SEKV_MAX_SPAN_LEN (sekv_build_sizes returns
+ *   UNSUPPORTED there), else 0.
+ *   stream: cudaStream_t of the CURRENT device (0 = default stream).  Asynchronous: outputs are ready when the
+ *   stream reaches the end of this call's work.
+ * Errors: INVALID_ARG (NULL pointer, bad cfg / offsets) and UNSUPPORTED ("... exceeds SEKV_STATIC_MAX_...", nothing
+ * launched, outputs untouched) -- the message is returned by sekv_static_last_error().  CUDA for launch failures.
+ * Every call on a device shares that device's array, which keeps the previous call's contents (this call needs
+ * nothing pre-zeroed beyond what it clears itself): calls that overlap on the GPU -- two streams, or two threads --
+ * RACE; serialise them (same stream, or an event between them). */
+#define SEKV_STATIC_MAX_TOKENS (1 << 20)
+#define SEKV_STATIC_MAX_SEQS 1024
+SEKV_API sekv_status sekv_segment_counts_static(const sekv_config* cfg, int32_t n_seqs, const int64_t* seq_tok_off,
+                                                const float* H, int32_t* counts, int32_t* too_long, void* stream);
+/* Message of the calling thread's last failed sekv_segment_counts_static call ("" if none). */
+SEKV_API const char* sekv_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -108,7 +108,10 @@ def _load() -> C.CDLL:
     lib.sekv_get_path.argtypes = [VP, P(I32), P(C.c_char_p)]
     lib.sekv_graph_count.argtypes = [VP, P(I32)]
     lib.sekv_export_span_factors.argtypes = [VP, I32, I32, I32, I32, P(I32), P(I32), P(I32), VP, VP, VP, VP, VP, VP, P(I32)]
-    for name in ("sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
+    lib.sekv_segment_counts_static.argtypes = [P(sekv_config), I32, P(I64), VP, VP, VP, VP]
+    lib.sekv_static_last_error.restype = C.c_char_p
+    lib.sekv_static_last_error.argtypes = []
+    for name in ("sekv_segment_counts_static", "sekv_device_arena_bytes", "sekv_create", "sekv_build_spans", "sekv_build_spans_prefactored",
                  "sekv_reset", "sekv_route", "sekv_decode_attn", "sekv_decode_step", "sekv_decode_step_host",
                  "sekv_last_zoom_ids",
                  "sekv_get_layout", "sekv_get_stats", "sekv_reset_stats", "sekv_cache_flush",
@@ -156,6 +159,28 @@ def sekv_build_sizes(cfg: sekv_config, seq_tok_off: Sequence[int], H: Optional[t
     if st != SEKV_OK:
         raise SekvError(st, "sekv_build_sizes")
     return out, list(spans), list(pool)
+
+
+SEKV_STATIC_MAX_TOKENS = 1 << 20
+SEKV_STATIC_MAX_SEQS = 1024
+
+
+def sekv_segment_counts_static(cfg: sekv_config, seq_tok_off: Sequence[int], H: torch.Tensor, counts: torch.Tensor,
+                               too_long: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """Per-sequence (pool tokens, spans) into the DEVICE int32 tensor counts [n_seqs, 2] and the span-too-long flag into
+    the DEVICE int32 tensor too_long [1], on scratch the library holds in a static device array: nothing is allocated
+    (include/sekv.h).  Asynchronous on `stream` (default: torch's current stream)."""
+    n = len(seq_tok_off) - 1
+    off = (C.c_int64 * (n + 1))(*[int(x) for x in seq_tok_off])
+    assert H.is_cuda and H.dtype == torch.float32 and H.is_contiguous()
+    assert counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous() and counts.numel() >= 2 * n
+    assert too_long.is_cuda and too_long.dtype == torch.int32 and too_long.numel() >= 1
+    s = stream if stream is not None else torch.cuda.current_stream(H.device)
+    with torch.cuda.device(H.device):
+        st = lib.sekv_segment_counts_static(C.byref(cfg), n, off, H.data_ptr(), counts.data_ptr(), too_long.data_ptr(),
+                                            s.cuda_stream)
+    if st != SEKV_OK:
+        raise SekvError(st, "sekv_segment_counts_static: " + lib.sekv_static_last_error().decode())
 
 
 def make_config(**kw) -> sekv_config:

@@ -483,3 +483,72 @@ cudaError_t launch_build_dense(sekv_handle* h, int layer, const float* H, const 
 }
 
 }  // namespace sekv
+
+// ---------------------------------------------------------------------------------------------
+// sekv_segment_counts_static (include/sekv.h): the four scan kernels of the segmentation rule on scratch that
+// is NOT allocated: a file-scope device array.  In host code `g_static_scratch` is only a stand-in for the
+// symbol, not a device address; the address a kernel can use comes from cudaGetSymbolAddress, looked up once
+// per device (with that device current) and kept in g_static_ptr.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kStOffFlag = 0;                                                   // uint8 [tokens]
+constexpr size_t kStOffFlag2 = kStOffFlag + (size_t)SEKV_STATIC_MAX_TOKENS;         // uint8 [tokens]
+constexpr size_t kStOffLen = kStOffFlag2 + (size_t)SEKV_STATIC_MAX_TOKENS;          // int32 [tokens]
+constexpr size_t kStOffTok = kStOffLen + (size_t)SEKV_STATIC_MAX_TOKENS * 4;        // int64 [seqs + 1]
+constexpr size_t kStOffThr = kStOffTok + (((size_t)SEKV_STATIC_MAX_SEQS + 1) * 8 + 255) / 256 * 256;   // double [seqs]
+constexpr size_t kStBytes = kStOffThr + (size_t)SEKV_STATIC_MAX_SEQS * 8;
+static_assert(kStOffLen % 256 == 0 && kStOffTok % 256 == 0 && kStOffThr % 256 == 0, "scratch alignment");
+
+static __device__ __align__(256) uint8_t g_static_scratch[kStBytes];
+
+constexpr int kStMaxDevices = 64;
+uint8_t* g_static_ptr[kStMaxDevices];              // device address of g_static_scratch per device (null: not looked up)
+thread_local const char* g_static_err = "";
+
+sekv_status static_fail(sekv_status st, const char* msg) { g_static_err = msg; return st; }
+
+}  // namespace
+
+extern "C" const char* sekv_static_last_error(void) { return g_static_err; }
+
+extern "C" sekv_status sekv_segment_counts_static(const sekv_config* cfg, int32_t n_seqs, const int64_t* seq_tok_off,
+                                                  const float* H, int32_t* counts, int32_t* too_long, void* stream) {
+  using namespace sekv;
+  if (!cfg || !seq_tok_off || !H || !counts || !too_long) return static_fail(SEKV_INVALID_ARG, "NULL argument");
+  if (n_seqs < 1) return static_fail(SEKV_INVALID_ARG, "n_seqs < 1");
+  if (cfg->l_min < 1 || cfg->window < 0 || !(cfg->alpha == cfg->alpha))
+    return static_fail(SEKV_INVALID_ARG, "bad cfg (l_min < 1, window < 0 or alpha is NaN)");
+  if (n_seqs > SEKV_STATIC_MAX_SEQS)
+    return static_fail(SEKV_UNSUPPORTED, "n_seqs exceeds SEKV_STATIC_MAX_SEQS (1024): use sekv_build_sizes");
+  if (seq_tok_off[0] != 0) return static_fail(SEKV_INVALID_ARG, "seq_tok_off[0] != 0");
+  for (int b = 0; b < n_seqs; ++b)
+    if (seq_tok_off[b + 1] <= seq_tok_off[b]) return static_fail(SEKV_INVALID_ARG, "seq_tok_off is not increasing");
+  if (seq_tok_off[n_seqs] > (int64_t)SEKV_STATIC_MAX_TOKENS)
+    return static_fail(SEKV_UNSUPPORTED, "token count exceeds SEKV_STATIC_MAX_TOKENS (1048576): use sekv_build_sizes");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return static_fail(SEKV_CUDA, "cudaGetDevice failed"); }
+  if (dev < 0 || dev >= kStMaxDevices) return static_fail(SEKV_UNSUPPORTED, "device ordinal >= 64");
+  uint8_t* base = g_static_ptr[dev];
+  if (base == nullptr) {                    // first call on this device (racing threads store the same value)
+    void* p = nullptr;
+    const cudaError_t ge = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (ge != cudaSuccess || p == nullptr) {
+      cudaGetLastError();
+      return static_fail(SEKV_CUDA, "cudaGetSymbolAddress of the static scratch failed");
+    }
+    base = g_static_ptr[dev] = (uint8_t*)p;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  // (pageable host memory is staged before cudaMemcpyAsync returns: the caller's array may be reused at once)
+  cudaError_t e = cudaMemcpyAsync(base + kStOffTok, seq_tok_off, (size_t)(n_seqs + 1) * 8, cudaMemcpyHostToDevice, s);
+  // segment_scan clears *too_long itself; every other scratch byte a kernel reads was written by an earlier kernel
+  // of this call (flags for every token, run lengths at the span starts that are read back), so the previous
+  // call's contents are never seen
+  if (e == cudaSuccess)
+    e = segment_scan(H, n_seqs, (const int64_t*)(base + kStOffTok), (double)cfg->alpha, cfg->window, cfg->l_min,
+                     SEKV_MAX_SPAN_LEN, base + kStOffFlag, base + kStOffFlag2, (int32_t*)(base + kStOffLen),
+                     (double*)(base + kStOffThr), counts, too_long, s);
+  if (e != cudaSuccess) { cudaGetLastError(); return static_fail(SEKV_CUDA, cudaGetErrorString(e)); }
+  return SEKV_OK;
+}
