@@ -78,3 +78,76 @@ def test_degenerate_sequences_in_one_batch(impl):
             assert rel_l2(got, ref) <= TOL_BF16["rel_l2"], (b, rel_l2(got, ref))
             assert float(np.abs(got - ref).max()) <= TOL_BF16["max_abs"]
     eng.close()
+
+
+def _max_span_spec(n_spans):
+    # spans of exactly L_min = 16 tokens, two anchors after each (the last span takes the two leftover tokens too)
+    return get_spec(1).sharp().with_(contexts=(18 * n_spans,), len_lo=16, len_hi=16, anchors_per_span=2)
+
+
+def test_maximum_spans_per_sequence():
+    """SEKV_MAX_SPANS_PER_SEQ = 8192 spans in ONE sequence (the most the span tables of a sequence hold): routing over
+    8192 summaries per head and the top-k select over them, attention with 16 of them expanded."""
+    from paper_2606_31145_b200 import engine as E
+    from paper_2606_31145_b200.export import export_tables
+    spec = _max_span_spec(8192)
+    lay = make_layouts(spec)
+    assert lay[0].m == 8192 and lay[0].A == 2 * 8191
+    eng = E.create_engine(spec, lay, gen_device="cuda", prefetch=4)
+    fused, why = eng.sekv_get_path()
+    print("8192 spans: fused =", bool(fused), why)
+    T = tables_from_export(export_tables(eng, 0, 0, True), spec.n_q_heads, spec.n_kv_heads, spec.route_dim)
+    assert T.seg.m == 8192
+    q = make_queries(spec, 0, "cuda")[0]
+    ids, count, _ = compare_route(eng, 0, q, spec.top_k, [T])
+    _, worst = compare_attn(eng, 0, q, ids, count, [T], TOL_BF16, heads=[0, 9, 22, 31])
+    out = torch.zeros((1, 1, spec.n_q_heads, 128), dtype=eng.out_dtype, device="cuda")
+    eng.sekv_decode_step(q[None].contiguous(), spec.top_k, out)
+    torch.cuda.synchronize()
+    ids2, count2 = eng.sekv_last_zoom_ids(0)
+    zoom = [[int(x) for x in ids2[0, g, :int(count2[0, g])].cpu().numpy()] for g in range(spec.n_kv_heads)]
+    ref, _ = O.decode_attn(to_np(q)[0], T, zoom, heads=[0, 9, 22, 31])
+    got = out[0, 0].float().cpu().numpy()
+    assert rel_l2(got[[0, 9, 22, 31]], ref[[0, 9, 22, 31]]) <= TOL_BF16["rel_l2"]
+    print("8192 spans", worst)
+    eng.close()
+
+
+def test_one_span_more_than_the_maximum_is_refused():
+    from paper_2606_31145_b200 import binding as B
+    from paper_2606_31145_b200 import engine as E
+    spec = _max_span_spec(8193)
+    lay = make_layouts(spec)
+    assert lay[0].m == 8193
+    with pytest.raises(B.SekvError) as ei:
+        E.create_engine(spec, lay, gen_device="cuda", prefetch=4)
+    assert ei.value.status in (B.SEKV_UNSUPPORTED, B.SEKV_INVALID_ARG) and "8192" in str(ei.value)
+
+
+def test_maximum_span_length_and_rank():
+    """Spans of SEKV_MAX_SPAN_LEN = 1024 tokens with rank SEKV_MAX_RANK = 64 factors (the largest blob the store
+    holds: 289 KB, read in many windows), 28 / 4 heads (G = 7), the first step with every expansion a demand miss."""
+    from paper_2606_31145_b200 import engine as E
+    from paper_2606_31145_b200.export import export_tables
+    spec = get_spec(4, rank=64, top_k=8).sharp().with_(contexts=(20 * 1028 - 4,), len_lo=1024, len_hi=1024)
+    lay = make_layouts(spec)
+    assert lay[0].m == 20 and int(lay[0].planted_span_len.min()) == 1024 and int(lay[0].planted_span_len.max()) == 1024
+    eng = E.create_engine(spec, lay, gen_device="cuda", prefetch=2)
+    fused, why = eng.sekv_get_path()
+    assert fused, why
+    T = tables_from_export(export_tables(eng, 0, 0, True), spec.n_q_heads, spec.n_kv_heads, spec.route_dim)
+    q = make_queries(spec, 0, "cuda")[0]
+    ids, count, _ = compare_route(eng, 0, q, spec.top_k, [T])
+    out = torch.zeros((1, 1, spec.n_q_heads, 128), dtype=eng.out_dtype, device="cuda")
+    for step in range(2):                       # step 0: all demand misses (host store over PCIe), step 1: all hits
+        eng.sekv_decode_step(q[None].contiguous(), spec.top_k, out)
+        torch.cuda.synchronize()
+        ids2, count2 = eng.sekv_last_zoom_ids(0)
+        zoom = [[int(x) for x in ids2[0, g, :int(count2[0, g])].cpu().numpy()] for g in range(spec.n_kv_heads)]
+        ref, _ = O.decode_attn(to_np(q)[0], T, zoom)
+        got = out[0, 0].float().cpu().numpy()
+        assert rel_l2(got, ref) <= TOL_BF16["rel_l2"], (step, rel_l2(got, ref))
+        assert float(np.abs(got - ref).max()) <= TOL_BF16["max_abs"]
+    st = eng.sekv_get_stats()
+    assert st["cache_misses"] >= 8 * spec.n_kv_heads and st["cache_hits"] >= 8 * spec.n_kv_heads
+    eng.close()
