@@ -29,7 +29,9 @@ def config_for(spec, layouts, *, k_cap: Optional[int] = None, cache_ways: Option
     if spec.top_k < 0:
         prefetch = 0
     if cache_ways is None:
-        cache_ways = max(2 * (k_cap + prefetch), 1) if spec.top_k >= 0 else max(k_cap, 1)
+        # SURVEY.md 8(c) reading 22: 4 x the per-step working set (and never fewer than two steps' zoom sets plus
+        # prefetch candidates); at configs[2] that is 128 slots, inside the paper's 10% budget (L123)
+        cache_ways = max(4 * k_cap, 2 * (k_cap + prefetch), 1) if spec.top_k >= 0 else max(k_cap, 1)
     cfg = B.make_config(
         **base, max_tokens_total=sz.tokens_total, max_spans_total=int(sz.spans_total * slack) + 1,
         max_full_total=int(sz.full_total * slack) + 1, max_span_len=min(1024, -(-max(sz.max_span_len, 16) // 16) * 16),
