@@ -205,11 +205,13 @@ __device__ __forceinline__ void qproj_mma(const FusedParams& P, int hl, int j0, 
 }
 
 // meta = |S| << 16 | rank_k | rank_v << 8 of the span
-// it = way | miss << 31 | no-slot << 30; j = index of the span in the sorted zoom list (the ZOOM item's partial slot)
+// it = way | miss << 31 | no-slot << 30 | way-pending << 29 (a demand miss whose slot the plan has not chosen yet: the
+// ZOOM item starts the fetch from the host store and reads `it` from P.zway[j] when it needs the slot);
+// j = index of the span in the sorted zoom list (the ZOOM item's partial slot; < 2^15)
 __device__ __forceinline__ void write_zdesc(const FusedParams& P, ZDescG* zd, int bg, int g, int span0, int id, uint32_t it,
                                             uint32_t meta, uint32_t epoch, int j = 0) {
   ZDescG d;
-  d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = (it & 0xC0003FFFu) | ((uint32_t)j << 14); d.id = id;
+  d.src = 0ull; d.bytes = 0u; d.len_rr = 0u; d.way_miss = (it & 0xE0003FFFu) | (((uint32_t)j & 0x7FFFu) << 14); d.id = id;
   d.epoch0 = epoch; d.epoch1 = epoch;
   if (id >= 0) {
     const int gs = span0 + id;
@@ -503,6 +505,10 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T_in
     // being given slots; a resident prefetch candidate needs no copy
     if (zoom && (way >= 0 || id < 0))
       write_zdesc(P, zd + (K - 1 - atomicAdd(pos_hit, 1)), bg, g, span0, id, (uint32_t)max(way, 0), meta, epoch, j);
+    // ... and so do the demand misses, before their slot is known: their blob crosses PCIe (the longest pole of the
+    // layer at a few misses per step), and the fetch needs the slot only when the first bytes have arrived
+    if (zoom && id >= 0 && way < 0)
+      write_zdesc(P, zd + atomicAdd(pos_miss, 1), bg, g, span0, id, 0xA0000000u, meta, epoch, j);
   }
   int n_need;
   team_excl_scan(T, n_miss + n_pf, &n_need);                   // (its barriers also publish pass 1 to the team)
@@ -590,7 +596,7 @@ __device__ __forceinline__ void plan_team(const FusedParams& P, const Team& T_in
       items[j] = it;
     }
     miss_base += tot;
-    if (miss && j < n_zoom) write_zdesc(P, zd + atomicAdd(pos_miss, 1), bg, g, span0, id, it, t.meta[id], epoch, j);
+    if (miss && j < n_zoom) P.zway[(size_t)bg * P.kc + j] = make_uint2(it, epoch);      // the slot of demand miss j (self-validating pair)
   }
   team_bar(T);
   for (int w = T.tt; w < ways; w += T.ts) { tags[w] = t.sh_tag[w]; stamps[w] = t.sh_stamp[w]; }
@@ -1236,13 +1242,11 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
     // of host memory turn into many 32-byte PCIe reads): first the header into the front of the region (and on into
     // the slot, when the plan gave it one), then the chunk windows behind it, each kept in the slot on the way.
     const bool miss = (d.way_miss & 0x80000000u) != 0u;
-    uint8_t* wb = nullptr;
-    if ((d.way_miss & 0xC0000000u) == 0x80000000u) wb = P.lv.slots + ((size_t)bg * P.ways + (d.way_miss & 0x3FFFu)) * P.slot_bytes;
     const uint32_t hdr_bytes = (uint32_t)(nks + nvs) * (64u + 4096u), chunk_bytes = (uint32_t)(nks + nvs) * 512u;
     const uint8_t* hdr = blob;
     uint8_t* cbase = region;
     uint32_t cap = (uint32_t)P.region_bytes;
-    bool hdr_smem = false, wb_regs = wb != nullptr;
+    bool hdr_smem = false;
     uint64_t* hbar = nullptr;
     if (miss && hdr_bytes + chunk_bytes <= (uint32_t)P.region_bytes) {
       __syncwarp();
@@ -1251,9 +1255,26 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
         bulk_g2s(region, blob, hdr_bytes, bar + 1);
       }
       hbar = bar + 1;
-      hdr = region; hdr_smem = true; wb_regs = false;
+      hdr = region; hdr_smem = true;
       cbase = region + hdr_bytes; cap = (uint32_t)P.region_bytes - hdr_bytes;
     }
+    // the slot of a demand miss (the header is already on its way): chosen by the plan a little after the descriptor
+    uint8_t* wb = nullptr;
+    if (miss) {
+      uint32_t it = d.way_miss;
+      if (it & 0x20000000u) {
+        const uint2* zw = P.zway + (size_t)bg * P.kc + ((d.way_miss >> 14) & 0x7FFFu);
+        uint2 w;
+        for (;;) {
+          asm volatile("ld.relaxed.gpu.global.v2.u32 {%0,%1}, [%2];" : "=r"(w.x), "=r"(w.y) : "l"(zw) : "memory");
+          if (w.y == epoch) break;
+          __nanosleep(64);
+        }
+        it = w.x;
+      }
+      if ((it & 0xC0000000u) == 0x80000000u) wb = P.lv.slots + ((size_t)bg * P.ways + (it & 0x3FFFu)) * P.slot_bytes;
+    }
+    const bool wb_regs = wb != nullptr && !hdr_smem;
     if (nks <= 1 && nvs <= 1)
       zoom_span<G, 1>(P, blob, hdr, hdr_smem, len, 1, 1, cbase, cap, bar, phase, lane, qf, M, L, of, wb, wb_regs, hbar, &phase1, hdr_bytes, tm);
     else
@@ -1264,7 +1285,7 @@ __device__ __forceinline__ void zoom_item(const FusedParams& P, const Item& I, u
   }
   mark(tm, 3, lane);
   Item Ij = I;                                                   // the partial of list index j goes to slot j
-  Ij.part = I.part - I.a + (int)((d.way_miss >> 14) & 0xFFFFu);
+  Ij.part = I.part - I.a + (int)((d.way_miss >> 14) & 0x7FFFu);
   store_partial<G>(P, Ij, lane, M, L, of);
   __syncwarp();
   if (lane == 0) red_add_release(grp_ctr(ctrs, bg), kAttnOne);
@@ -1724,6 +1745,7 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   P.route_head_stride = (size_t)h->lay.spans_cap * c.route_dim;
   if (!fused_geometry(h, &P, nullptr)) return cudaErrorInvalidConfiguration;
   P.zmask2 = (uint2*)ws(h, h->F.off_zmask2) + (size_t)layer * c.max_seqs * c.n_kv_heads * h->mask_words;
+  P.zway = (uint2*)ws(h, h->F.off_zway) + (size_t)layer * c.max_seqs * c.n_kv_heads * (std::max(c.k_cap, 1) + std::max(c.prefetch, 0));
   // the chain (a1-a4) runs whenever there is routing to do or a zoom set to plan
   P.has_chain = ((mode & FM_ROUTE) || c.k_cap > 0) ? 1 : 0;
   // layers 1.. of a whole-step launch: the kernel before this one on the stream is the previous layer's of the same

@@ -112,6 +112,7 @@ void compute_layout(const sekv_config& c, FullLayout* F) {
   F->off_bg_route = cv.take((size_t)(B * Hkv) * 4);
   F->ctrs_per_layer = (int)(4 + 2 * (4 + 4 * B * Hkv));       // sequence number + two counter sets
   F->off_zdesc = cv.take((size_t)NL * B * Hkv * kc * sizeof(ZDescG));
+  F->off_zway = cv.take((size_t)NL * B * Hkv * kc * sizeof(uint2));
   F->off_zmask2 = cv.take((size_t)NL * B * Hkv * F->mask_words * 8);
   F->off_ctrs = cv.take((size_t)NL * F->ctrs_per_layer * 4);
   F->off_plan_counts = cv.take((size_t)NL * B * Hkv * 2 * 4);
@@ -379,6 +380,8 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_layer_step, 0, (size_t)c.n_layers * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zdesc, 0, (size_t)c.n_layers * c.max_seqs * c.n_kv_heads *
                         (std::max(c.k_cap, 1) + std::max(c.prefetch, 0)) * sizeof(ZDescG), h->main));   // stamps restart
+  CK(h, cudaMemsetAsync(h->dev + F.off_zway, 0, (size_t)c.n_layers * c.max_seqs * c.n_kv_heads *
+                        (std::max(c.k_cap, 1) + std::max(c.prefetch, 0)) * sizeof(uint2), h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_stats, 0, ST_COUNT * 8, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zoom_mask, 0, (size_t)regions * F.mask_words * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_zmask2, 0, (size_t)regions * F.mask_words * 8, h->main));      // stamps restart

@@ -159,7 +159,7 @@ struct __align__(16) ZDescG {   // what a ZOOM item needs to know about one expa
   uint32_t bytes;
   uint32_t epoch0;              // the layer's step stamp: both halves carry it, ZOOM items poll until it matches
   uint32_t len_rr;              // |S| << 16 | rank_k | rank_v << 8
-  uint32_t way_miss;            // way | miss << 31 | no-slot << 30
+  uint32_t way_miss;            // way | j << 14 | way-pending << 29 | no-slot << 30 | miss << 31
   int32_t id;                   // local span id, -1 = dropped duplicate
   uint32_t epoch1;
 };
@@ -193,6 +193,7 @@ struct FusedParams {
   size_t ent_head_stride, route_head_stride;
   int64_t slot_bytes, trace_cap;
   uint2* zmask2;               // [BG][mask_words] (zoom bits, step stamp) pairs of this layer
+  uint2* zway;                 // [BG][kc] (it, step stamp) of the demand misses of this layer: their slot, published after the descriptor
   int32_t main_end;                              // number of work items of this launch
   int32_t mode, k, k_cap, prefetch, kc, BG;
   int32_t Hq, Hkv, dp, ways, mask_words, spans_cap, m_tot, out_bf16;
@@ -258,7 +259,7 @@ struct FullLayout {
   int64_t off_partials1, off_partials2, off_ws_ids, off_ws_count, off_stats, off_chunks, off_bg_chunk,
       off_zoom_mask, off_items, off_item_span, off_layer_step, off_seg_flag, off_seg_flag2, off_seg_len,
       off_seg_misc, off_q_stage, off_out_stage, off_lse_stage, off_err_flag, off_items_sched, off_bg_part,
-      off_bg_route, off_ctrs, off_plan_counts, off_zdesc, off_zmask2;
+      off_bg_route, off_ctrs, off_plan_counts, off_zdesc, off_zmask2, off_zway;
   int mask_words, max_chunks, max_items, ctrs_per_layer;
   size_t total;
 };
