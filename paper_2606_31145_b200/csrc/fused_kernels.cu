@@ -1436,13 +1436,22 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
   uint32_t epoch = 0u;
   int idx = -1;
   Item first;
-  bool prefilled = false;
+  bool prefilled = false, pf_done = false;
   if (!is_team) {
     const int b = (int)blockIdx.x;
     idx = chain_cta ? b * (nw - ntw) + (warp - ntw) : n_chain_cta * (nw - ntw) + (b - n_chain_cta) * nw + warp;
     if (idx < P.main_end) {
       first = load_item(P.items + idx);
       if (first.kind == IT_POOL) { rows_prefill(P, first, region, lane); prefilled = true; }
+      // P.pf_early: the prefetch candidates this launch copies are those of the layer TWO launches back.  That launch is
+      // complete whenever a CTA of this one runs: the grid holds one CTA per SM, so this CTA got its SM from a CTA of
+      // the previous launch that has exited, i.e. that passed its own dependency wait.  The copy therefore runs here,
+      // BEFORE the wait, while this SM has nothing else to do: a copy from the host store in flight slows the SM's
+      // other memory traffic down (a pool item next to one took 16 us instead of 10, profiles/r02_item_trace.md).
+      if (first.kind == IT_PREFETCH && P.pf_early) {
+        if (P.pf_plan_counts != nullptr) prefetch_item(P, first, region, bar, phase, lane);
+        pf_done = true;
+      }
     }
   }
   // The layer's step stamp and launch sequence number (which picks the counter set) are only written by launches
@@ -1510,7 +1519,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
         case IT_POOL:
         case IT_COARSE: rows_item<G>(P, cur, region, lane, epoch, ctrs, ah, prefilled, tm); prefilled = false; break;
         case IT_ZOOM: zoom_item<G>(P, cur, region, bar, phase, phase1, lane, epoch, ctrs, tm); break;
-        case IT_PREFETCH: if (P.pf_plan_counts != nullptr) prefetch_item(P, cur, region, bar, phase, lane); break;
+        case IT_PREFETCH: if (P.pf_plan_counts != nullptr && !pf_done) prefetch_item(P, cur, region, bar, phase, lane); pf_done = false; break;
         default: combine_item(P, cur, region, bar, phase, lane, ctrs, tm); break;
       }
       if (P.trace && lane == 0 && cur_idx < P.trace_cap) {
@@ -1731,7 +1740,10 @@ cudaError_t launch_fused(sekv_handle* h, int layer, int mode, const void* q, con
   // l + 1 (those of the last layer by layer 0 of the next step; sekv_api.cu covers the cases without one).
   if (!((mode & FM_ROUTE) && (mode & FM_ATTN))) P.prefetch = 0;
   if ((mode & FM_ROUTE) && (mode & FM_ATTN) && c.n_layers > 1 && c.prefetch > 0 && c.k_cap > 0) {
-    const int pl = (layer + c.n_layers - 1) % c.n_layers;       // layer 0 carries the last layer's copies of the previous step
+    // with three layers or more: the layer two launches back, copied before the dependency wait (fused_layer_kernel);
+    // layers 0 and 1 carry the last two layers' copies of the previous step
+    P.pf_early = c.n_layers >= 3 ? 1 : 0;
+    const int pl = (layer + c.n_layers - (P.pf_early ? 2 : 1)) % c.n_layers;
     P.pf_lv = layer_view(h, pl);
     P.pf_plan_counts = (const int32_t*)ws(h, h->F.off_plan_counts) + (size_t)pl * c.max_seqs * c.n_kv_heads * 2;
   }

@@ -389,7 +389,7 @@ sekv_status sekv_reset(sekv_handle* h) {
   CK(h, cudaMemsetAsync(h->dev + F.off_ctrs, 0, (size_t)c.n_layers * F.ctrs_per_layer * 4, h->main));
   CK(h, cudaMemsetAsync(h->dev + F.off_plan_counts, 0, (size_t)regions * 2 * 4, h->main));
   CK(h, cudaStreamSynchronize(h->main));
-  h->pending_prefetch = -1;
+  h->pending_prefetch = -1; h->pending_prefetch2 = -1;
   h->n_items = 0; h->use_fused = false; h->fused_why = "no sequences built";
   h->n_seqs = 0; h->segmented = false; h->m_b.clear(); h->A_b.clear(); h->tok_off.clear();
   h->span_len_host.clear();
@@ -804,9 +804,9 @@ static cudaError_t decode_layer(sekv_handle* h, int layer, const void* q, const 
                                 void* out, float* lse) {
   cudaError_t e;
   if (h->use_fused) {     // caller-supplied zoom set: plan + attention + combine in the fused layer kernel
-    if (h->pending_prefetch == layer) {     // this layer's cache is about to be read: finish its prefetch copies first
+    if (h->pending_prefetch == layer || h->pending_prefetch2 == layer) {   // this layer's cache is about to be read: finish its prefetch copies first
       if ((e = launch_prefetch(h, layer, h->main)) != cudaSuccess) return e;
-      h->pending_prefetch = -1;
+      if (h->pending_prefetch == layer) h->pending_prefetch = -1; else h->pending_prefetch2 = -1;
     }
     ProfScope ps(h, 6, h->main);
     return launch_fused(h, layer, FM_ATTN, q, nullptr, 0, nullptr, nullptr, (int32_t*)ids, (int32_t*)count, out, lse, h->main);
@@ -932,8 +932,11 @@ static sekv_status decode_step_impl(sekv_handle* h, const void* q, const float* 
 sekv_status sekv_decode_step(sekv_handle* h, const void* q, const float* tau, int32_t k, void* out, float* lse) {
   const sekv_status s = decode_step_impl(h, q, tau, k, out, lse);
   // the last layer's prefetch candidates are copied by layer 0 of the next step (or before the next read of its cache)
-  if (s == SEKV_OK && h->use_fused && h->cfg.k_cap > 0 && h->cfg.prefetch > 0 && k >= 0)
+  if (s == SEKV_OK && h->use_fused && h->cfg.k_cap > 0 && h->cfg.prefetch > 0 && k >= 0) {
     h->pending_prefetch = h->cfg.n_layers - 1;
+    // (three layers or more: a layer's candidates are copied two launches later, fused_kernels.cu)
+    h->pending_prefetch2 = h->cfg.n_layers >= 3 ? h->cfg.n_layers - 2 : -1;
+  }
   return s;
 }
 

@@ -184,6 +184,7 @@ struct FusedParams {
   int32_t* plan_counts;        // [BG][2] = n_zoom, n_cand
   LayerView pf_lv;             // the previous layer of the step: its prefetch candidates are copied by this launch
   const int32_t* pf_plan_counts;   // (null: nothing to copy)
+  int32_t pf_early;                // pf_lv is the layer two launches back: its copies run before the dependency wait
   unsigned long long* stats;
   const uint8_t* host_arena;   // device alias of the pinned host factor store
   unsigned long long* trace;   // null, or 8 x u64 per item (sekv_set_trace)
@@ -295,6 +296,7 @@ struct sekv_handle {
   std::vector<GraphEntry> graphs;
   uint64_t launches;
   int pending_prefetch;              // layer whose speculative prefetch copies have not been carried out yet (-1: none)
+  int pending_prefetch2;             // a second such layer (the one before it), or -1
   // per-kernel-class CUDA-event timing (sekv_set_profiling)
   bool profiling;
   void* trace_buf; int64_t trace_cap;
