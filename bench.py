@@ -481,7 +481,7 @@ def run_ours(args):
                   "misses_per_step": st["cache_misses"] / args.steps, "zoomed_per_step": st["zoomed_spans"] / args.steps,
                   "value_at_100pct_hits": value_all_hits,
                   "fetch_exposed_us": (us_layer_step - value_all_hits) if value_all_hits is not None else None,
-                  "overlap": "demand misses are read by the bulk-copy engine inside the layer kernel; the speculative prefetch of layer l is copied inside layer l+1's kernel"},
+                  "overlap": "demand misses are read by the bulk-copy engine inside the layer kernel; the speculative prefetch of layer l is copied inside layer l+2's kernel, before its dependency wait"},
         "sweep": sweep,
     }
     if cpu_baseline:
