@@ -84,8 +84,11 @@ typedef struct sekv_config {
   int32_t max_span_len;      /* <= SEKV_MAX_SPAN_LEN; longer runs make build fail UNSUPPORTED */
   int32_t k_cap;             /* max zoomed spans per (sequence, kv head) and step */
   int32_t cache_ways;        /* device factor-cache slots per (layer, sequence, kv head), >= k_cap + prefetch */
-  int32_t prefetch;          /* speculative prefetch depth: after each layer-step the `prefetch` next-best spans by
-                                routing score that are not resident are copied host -> cache on the side stream */
+  int32_t prefetch;          /* speculative prefetch depth: the `prefetch` next-best spans by routing score of a
+                                layer-step that are not resident are given a slot and copied host -> cache off the
+                                critical path: in sekv_decode_step by the layer kernel two launches later (before its
+                                dependency wait; one launch later with two layers), else by a copy kernel before the
+                                layer's cache is read again */
   int32_t stage1_ctas;       /* generic path: stage-1 grid; 0 = auto (multiple of the SM count) */
   int32_t item_rows;         /* fused path: entry rows per POOL work item, multiple of 16 (COARSE items: min(this, 64)); 0 = one round over the streaming warps */
   int32_t zoom_spans_per_item; /* reserved (the fused path runs one expanded span per ZOOM work item) */
@@ -138,9 +141,9 @@ typedef struct sekv_stats {
   uint64_t h2d_bytes;            /* DEMAND-miss factor bytes read from the pinned host store (Eq. 20) */
   uint64_t factor_bytes_algo;    /* sum over expansions of (r_K+r_V)(|S|+d_h) b + 4(r_K+r_V): Eq. 18 with fp32 sigma */
   uint64_t coarse_rows_skipped;  /* coarse entries replaced by their tokens (= zoomed_spans) */
-  uint64_t prefetched_spans;     /* blobs copied by the side-stream prefetch (only those that were given a slot) */
+  uint64_t prefetched_spans;     /* blobs copied by the speculative prefetch (only those that were given a slot) */
   uint64_t kernel_launches;      /* kernels launched or graph nodes replayed by this handle */
-  uint64_t prefetch_h2d_bytes;   /* bytes of the blobs copied by the speculative side-stream prefetch */
+  uint64_t prefetch_h2d_bytes;   /* bytes of the blobs copied by the speculative prefetch */
 } sekv_stats;
 
 /* Capacities a caller needs BEFORE sekv_create (sekv_build_sizes). */
@@ -283,7 +286,7 @@ SEKV_API sekv_status sekv_static_bytes_per_layer(const sekv_handle* h, uint64_t*
  * sekv_route / sekv_decode_attn / sekv_decode_step (non-graph launches only; a graph replay is not
  * instrumented).  Classes: 0 route (a1-a3), 1 plan (a4 residency), 2 fetch (a4 copy, side stream),
  * 3 stage 1 (a5), 4 stage 2 (a6), 5 combine (a7) -- the generic multi-kernel path -- and 6 the fused
- * layer kernel (a1-a7 in one launch, bf16 path), 7 the side-stream prefetch copy.
+ * layer kernel (a1-a7 in one launch, bf16 path), 7 the stand-alone prefetch copy kernel.
  * sekv_get_kernel_times synchronises, writes the summed milliseconds and launch counts per class since
  * the last call (HOST arrays of SEKV_N_KERNEL_CLASSES) and clears. */
 #define SEKV_N_KERNEL_CLASSES 8
