@@ -1505,12 +1505,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) fused_layer_kernel(const __g
   };
   if (is_team) idx = claim();
   if (idx < P.main_end) {
-    // Claims run ahead only through POOL and COARSE items (short or dependency-free: the claimed item does not wait
-    // long behind them).  Any other item is claimed when the warp is free to run it.
+    // Claims run ahead only through POOL items (dependency-free: the claimed item does not wait long behind them).
+    // Any other item is claimed when the warp is free to run it: a claim binds the item to this warp, and an item
+    // bound behind a COARSE or ZOOM item that is waiting for its chain starts later than it would on a free warp
+    // (measured: -0.7 us per layer-step at 100% hits against claiming ahead through COARSE items too).
     Item cur = is_team ? load_item(P.items + idx) : first;
     for (;;) {
       Ahead ah;
-      ah.on = cur.kind == IT_POOL || cur.kind == IT_COARSE; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
+      ah.on = cur.kind == IT_POOL; ah.done = false; ah.n_static = n_static; ah.pending = 0; ah.nidx = P.main_end;
       if (ah.on && lane == 0) ah.pending = atomicAdd(ctrs, 1);
       unsigned long long t0 = 0ull;
       const int cur_idx = idx;
