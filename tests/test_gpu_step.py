@@ -86,6 +86,41 @@ def test_step_prefetch_reduces_demand_misses():
     assert st1["cache_misses"] < st0["cache_misses"], (st0, st1)
 
 
+@pytest.mark.parametrize("use_graph", [0, 1])
+def test_step_four_layers_prefetch_two_launches_back(use_graph):
+    """Three layers or more: a layer's prefetch candidates are copied by the kernel two launches later, before its
+    dependency wait (layers 0 and 1 carry the last two layers' candidates of the previous step).  Every step of every
+    layer against the oracle; the copies must have landed (prefetched spans turn into hits: fewer demand misses than
+    without them), also after a caller reads the last two layers' caches between two steps (sekv_decode_attn on a
+    layer whose copies are still pending runs them first)."""
+    spec = get_spec(1).sharp().with_(n_layers=4, contexts=(18000,))
+    eng0, st0, _ = _run_steps(spec, 6, 0.9, heads=[0, 9, 31], prefetch=0, cache_ways=64, use_graph=use_graph)
+    eng0.close()
+    eng1, st1, worst = _run_steps(spec, 6, 0.9, heads=[0, 9, 31], prefetch=8, cache_ways=64, use_graph=use_graph)
+    print("step 4 layers", use_graph, worst, st0["cache_misses"], st1["cache_misses"], st1["prefetched_spans"])
+    assert st1["layer_steps"] == 24 and st1["prefetched_spans"] > 0
+    assert st1["cache_misses"] < st0["cache_misses"], (st0, st1)
+    # between two steps: attention on the last two layers with the zoom sets of the last step (all hits now)
+    from paper_2606_31145_b200.export import export_tables
+    from tests.gpu_common import compare_attn
+    q = make_queries(spec, 99, "cuda")
+    for l in (2, 3):
+        ids, count = eng1.sekv_last_zoom_ids(l)
+        T = tables_from_export(export_tables(eng1, l, 0), spec.n_q_heads, spec.n_kv_heads, spec.route_dim)
+        compare_attn(eng1, l, q[l], ids, count, [T], TOL_BF16, heads=[0, 9, 31])
+    out = torch.zeros((4, 1, spec.n_q_heads, 128), dtype=eng1.out_dtype, device="cuda")
+    eng1.sekv_decode_step(q, spec.top_k, out)
+    torch.cuda.synchronize()
+    qn = to_np(q)
+    for l in range(4):
+        ids, count = eng1.sekv_last_zoom_ids(l)
+        T = tables_from_export(export_tables(eng1, l, 0), spec.n_q_heads, spec.n_kv_heads, spec.route_dim)
+        zoom = [[int(x) for x in ids[0, g, :int(count[0, g])].cpu().numpy()] for g in range(spec.n_kv_heads)]
+        ref, _ = O.decode_attn(qn[l, 0], T, zoom, heads=[0, 9, 31])
+        assert rel_l2(out[l, 0].float().cpu().numpy()[[0, 9, 31]], ref[[0, 9, 31]]) <= TOL_BF16["rel_l2"], l
+    eng1.close()
+
+
 def test_step_ragged_batch_graph_replay():
     """Ragged batch (config 3, B = 3) through the CUDA-graph path: replays must see the new queries."""
     spec = get_spec(3, batch=3)
